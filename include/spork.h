@@ -1,0 +1,217 @@
+/*
+ * spork.h -- C ABI of libspork: the data-parallel hot path behind Spork's
+ * prefix-cache fork (arxiv/paper_2607_03333), B200 / sm_100a.
+ *
+ * What the paper fixes (PAPER.md = /root/reference/PAPER.md at build time):
+ *   - a probe is FORKED from the main stream so that its prompt prefix is a KV
+ *     cache hit ("Fork a completions request ... {D1 cache hit}", Algorithm 1
+ *     step 6; section 4.1);
+ *   - main and probe(s) DECODE concurrently over the shared prefix
+ *     (Fig. 7 text);
+ *   - D3 VERIFIES the k probe tokens as drafts "in the same decode step" and
+ *     accepts the longest greedy-matching prefix (section 4.3);
+ *   - a probe that ends / is rejected / times out / is superseded is RELEASED
+ *     (PAPER.md:211, :503, :585).
+ * The paper gives no mechanism below those events; the paged-KV design here
+ * (block tables, page refcounts, cascade split, LSE merge) follows
+ * BASELINE.json `north_star` and the readings A-1..A-25 in DESIGN.md.
+ *
+ * Conventions
+ *   - Every function returns 0 (SPORK_OK) or a negative spork error code.
+ *     Nothing throws or aborts across this boundary.
+ *   - "host" pointers are read (or written) before the call returns; the caller
+ *     may reuse them immediately.  "device" pointers are CUDA device memory,
+ *     caller-owned, used in stream order on `stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).
+ *   - All state-changing calls and attention calls on one handle must be issued
+ *     from one thread and onto one stream (or onto streams the caller orders).
+ *     A handle is not thread-safe.
+ *   - Batched state calls are all-or-nothing: on any error no state changes.
+ *   - The library never synchronises the stream on the success path, with two
+ *     documented exceptions: (a) when its lower bound on free pages cannot
+ *     prove that an allocating call fits, it reads the exact device-side free
+ *     count (one 4-byte copy); (b) the first attention call after a
+ *     fork/release/truncate reads back the per-group shared page counts.
+ *   - Page size is 16 tokens.  Page allocation is deterministic: the lowest
+ *     free page id first, requests in array order, positions ascending
+ *     (reading A-1), so block tables and refcounts are unique.
+ */
+#ifndef SPORK_H
+#define SPORK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPORK_PAGE_SIZE 16
+
+#define SPORK_OK 0
+#define SPORK_ERR_INVALID (-1)      /* bad argument / shape / unsupported config  */
+#define SPORK_ERR_OOM (-2)          /* not enough free pages (nothing changed)     */
+#define SPORK_ERR_NO_SLOT (-3)      /* not enough free sequence slots              */
+#define SPORK_ERR_TOO_LONG (-4)     /* sequence would exceed max_pages_per_seq     */
+#define SPORK_ERR_INVALID_SEQ (-5)  /* id out of range, not live, or repeated      */
+#define SPORK_ERR_SHARED (-6)       /* truncate would expose a shared partial page */
+#define SPORK_ERR_CUDA (-7)         /* a CUDA runtime call failed                  */
+#define SPORK_ERR_DEVICE (-8)       /* device-side consistency check tripped       */
+
+#define SPORK_F32 0
+#define SPORK_BF16 1
+
+typedef struct spork_ctx spork_ctx;
+
+typedef struct spork_config {
+    int32_t dtype;             /* SPORK_F32 | SPORK_BF16: storage type of K, V and Q    */
+    int32_t num_q_heads;       /* Hq                                                    */
+    int32_t num_kv_heads;      /* Hkv, divides Hq; q head h reads kv head h/(Hq/Hkv)    */
+    int32_t head_dim;          /* D: multiple of 32, <= 256                             */
+    int32_t page_size;         /* must be SPORK_PAGE_SIZE                               */
+    int32_t num_pages;         /* NP: pages in each pool                                */
+    int32_t max_seqs;          /* sequence slots                                        */
+    int32_t max_pages_per_seq; /* block-table row length                                */
+    float scale;               /* softmax scale (1/sqrt(D)); scores = scale * <q,k>     */
+} spork_config;
+
+/* Bytes of one page in ONE pool (K or V): Hkv * 16 * D * sizeof(dtype). */
+size_t spork_page_bytes(const spork_config *cfg);
+
+/*
+ * create / destroy.
+ * k_pool, v_pool: device, caller-owned (allocated with e.g. PyTorch), each
+ * num_pages * spork_page_bytes() bytes, 256-byte aligned, contents arbitrary.
+ * Logical layout of a pool is [num_pages][Hkv][16][D]; the arrangement of the
+ * 16 x D elements inside one (page, kv head) block is library-defined (for
+ * bf16 with D % 64 == 0 it is the 128-byte-swizzled shared-memory image the
+ * attention kernels consume, so a block is staged with one bulk copy).  Write
+ * pools only through spork_append / spork_fork; read them through
+ * spork_read_kv.  The library owns block tables, refcounts and workspace.
+ * Errors: SPORK_ERR_INVALID (shapes), SPORK_ERR_CUDA.
+ */
+int spork_create(const spork_config *cfg, void *k_pool, void *v_pool, spork_ctx **out);
+int spork_destroy(spork_ctx *ctx);
+
+/* n new empty sequences in the lowest free slots; ids_out: host int32[n]. */
+int spork_seq_create(spork_ctx *ctx, int n, int32_t *ids_out);
+
+/*
+ * append: the "prefill / decode wrote KV" event (Algorithm 1 steps 1-5,
+ * PAPER.md:257-261); also how draft KV is placed before verify.
+ * seq_ids, n_tokens: host int32[n] (a sequence may repeat; requests apply in
+ * array order).  k_src, v_src: device, [sum n_tokens][Hkv][D] in cfg.dtype.
+ * A page is allocated whenever a sequence crosses a page boundary.
+ * Errors: INVALID_SEQ, TOO_LONG, OOM.
+ */
+int spork_append(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t *n_tokens,
+                 const void *k_src, const void *v_src, void *stream);
+
+/*
+ * fork: Algorithm 1 step 6.  Child i clones parent_ids[i]'s
+ * block table: the floor(len/16) full pages are shared (refcount + 1 each),
+ * a partially filled tail page is duplicated into a fresh page (whole page,
+ * K and V), child length = parent length.  Parents must be live before the
+ * call; a parent may repeat.  Children take the lowest free slots in request
+ * order; child_ids_out: host int32[n].  The parent is unchanged.
+ * Errors: INVALID_SEQ, NO_SLOT, OOM.
+ */
+int spork_fork(spork_ctx *ctx, int n, const int32_t *parent_ids, int32_t *child_ids_out,
+               void *stream);
+
+/*
+ * release: the probe finished / was rejected / timed out / was superseded
+ * or the main stream finished.  Every block-table
+ * entry drops one reference; pages reaching 0 are free.  A parent may be
+ * released before its children.  Errors: INVALID_SEQ (not live, or repeated
+ * within the batch).
+ */
+int spork_release(spork_ctx *ctx, int n, const int32_t *seq_ids, void *stream);
+
+/*
+ * truncate: rollback of rejected drafts (section 4.3 step 3).
+ * new_len: host int32[n], 0 <= new_len <= len.  Frees whole pages beyond
+ * ceil(new_len/16).  Errors: INVALID_SEQ, INVALID, SHARED (the kept tail page
+ * is partially filled and has refcount > 1).
+ */
+int spork_truncate(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t *new_len,
+                   void *stream);
+
+/*
+ * decode attention, q_len = 1 (main and probes decode in one
+ * batch).  The batch is seq_ids[group_indptr[n_groups]] (host int32), split
+ * into fork groups by group_indptr (host int32[n_groups+1]); a group of 1 is
+ * plain paged decode.  For each group the library finds the longest run of
+ * leading pages common to all members and reads it from HBM once for the
+ * whole group (cascade); the result does not depend on the grouping beyond
+ * rounding.  q: device [n_seq][Hq][D] cfg.dtype.  out: device fp32
+ * [n_seq][Hq][D].  lse: device fp32 [n_seq][Hq], natural log of
+ * sum_t exp(scale * <q, k_t>).  Row i attends all len(seq_ids[i]) tokens; an
+ * empty sequence yields out = 0, lse = -inf.
+ * Errors: INVALID, INVALID_SEQ.
+ */
+int spork_decode_attn(spork_ctx *ctx, int n_groups, const int32_t *group_indptr,
+                      const int32_t *seq_ids, const void *q, float *out, float *lse,
+                      void *stream);
+
+/*
+ * verify attention (section 4.3 step 2): sequence i has
+ * k_i = q_indptr[i+1] - q_indptr[i] draft positions whose KV are already its
+ * last k_i tokens; query row j of sequence i attends tokens
+ * t <= len_i - k_i + j.  q: device [sum k][Hq][D]; out fp32 [sum k][Hq][D];
+ * lse fp32 [sum k][Hq].  Errors: INVALID (k_i < 1 or k_i > len_i), INVALID_SEQ.
+ */
+int spork_verify_attn(spork_ctx *ctx, int n_groups, const int32_t *group_indptr,
+                      const int32_t *seq_ids, const int32_t *q_indptr, const void *q,
+                      float *out, float *lse, void *stream);
+
+/*
+ * Host-buffer forms (what bench.py's `e2e` times): q_host, out_host, lse_host
+ * are HOST buffers (pinned for full speed); the copies run on `stream` inside
+ * the call, and the call returns after the results have landed.
+ */
+int spork_decode_attn_host(spork_ctx *ctx, int n_groups, const int32_t *group_indptr,
+                           const int32_t *seq_ids, const void *q_host, float *out_host,
+                           float *lse_host, void *stream);
+int spork_verify_attn_host(spork_ctx *ctx, int n_groups, const int32_t *group_indptr,
+                           const int32_t *seq_ids, const int32_t *q_indptr, const void *q_host,
+                           float *out_host, float *lse_host, void *stream);
+
+/* ---- synchronous export (parity checks; each call synchronises) ----------- */
+/* len_out: host int32 (-1 if the slot is not live); table_out: host
+ * int32[ceil(len/16)] read from the DEVICE block table. */
+int spork_export(spork_ctx *ctx, int32_t seq, int32_t *len_out, int32_t *table_out);
+/* host_out: host int32[num_pages], the device refcounts. */
+int spork_export_refcounts(spork_ctx *ctx, int32_t *host_out);
+/* logical K/V of tokens [t0, t0+n) of one sequence; k_out, v_out: HOST
+ * [n][Hkv][D] cfg.dtype. */
+int spork_read_kv(spork_ctx *ctx, int32_t seq, int32_t t0, int32_t n, void *k_out, void *v_out);
+/* device-side free page count (synchronises). */
+int spork_free_pages(spork_ctx *ctx, int32_t *out);
+/* synchronises and returns the sticky device error word (SPORK_OK if none). */
+int spork_status(spork_ctx *ctx);
+
+/* ---- introspection (bench / tests) --------------------------------------- */
+typedef struct spork_plan_info {
+    int32_t n_items;        /* work items of the last attention call                */
+    int32_t n_prefix_items; /* of which shared-prefix items                         */
+    int32_t chunk_tokens;   /* split-KV chunk length                                */
+    int32_t grid;           /* CTAs launched by the attention kernel                */
+    int32_t kernel;         /* 0 = simt (fp32 / generic), 1 = mma (bf16, D = 128)    */
+    int32_t plan_cached;    /* 1 if the last call reused the previous plan          */
+    int64_t unique_tokens;  /* sum_groups (shared + sum_members private) tokens     */
+    int64_t naive_tokens;   /* sum_members len                                      */
+    int64_t partial_rows;   /* rows of split-KV workspace written                   */
+    int32_t launches;       /* kernels launched by the last attention call          */
+    int32_t reserved;
+} spork_plan_info;
+int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
+/* kernels launched by the last state call (append / fork / release / truncate) */
+int spork_last_launches(spork_ctx *ctx);
+
+const char *spork_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPORK_H */

@@ -1,0 +1,309 @@
+"""paper_2607_03333_b200 -- Python binding of libspork (the C ABI in include/spork.h).
+
+Argument marshalling only: every step of the path (allocator, fork, append,
+release, cascade decode attention, verify attention, merge) runs in the CUDA
+kernels of libspork.so.  PyTorch is used for device memory and streams.  There
+is no CPU fallback: constructing a `Spork` without the built library or without
+a CUDA device raises.
+
+Method names mirror the ABI: seq_create, append, fork, release, truncate,
+decode_attn, verify_attn, export, export_refcounts, read_kv, status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+from . import build as _build
+
+F32, BF16 = 0, 1
+PAGE_SIZE = 16
+
+OK = 0
+ERR_INVALID, ERR_OOM, ERR_NO_SLOT, ERR_TOO_LONG, ERR_INVALID_SEQ, ERR_SHARED, ERR_CUDA, ERR_DEVICE = (
+    -1, -2, -3, -4, -5, -6, -7, -8)
+
+# every symbol include/spork.h declares (tests check that the library exports them all)
+ABI_SYMBOLS = [
+    "spork_page_bytes", "spork_create", "spork_destroy", "spork_seq_create", "spork_append",
+    "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
+    "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
+    "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
+    "spork_strerror",
+]
+
+
+class SporkConfig(C.Structure):
+    _fields_ = [("dtype", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
+                ("head_dim", C.c_int32), ("page_size", C.c_int32), ("num_pages", C.c_int32),
+                ("max_seqs", C.c_int32), ("max_pages_per_seq", C.c_int32), ("scale", C.c_float)]
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [("n_items", C.c_int32), ("n_prefix_items", C.c_int32), ("chunk_tokens", C.c_int32),
+                ("grid", C.c_int32), ("kernel", C.c_int32), ("plan_cached", C.c_int32),
+                ("unique_tokens", C.c_int64), ("naive_tokens", C.c_int64),
+                ("partial_rows", C.c_int64), ("launches", C.c_int32), ("reserved", C.c_int32)]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """dlopen libspork.so (building it first if needed) and declare the ABI signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build() if build_if_missing else _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError(f"libspork.so not found at {path}; run python -m paper_2607_03333_b200.build")
+    lib = C.CDLL(path)
+    P, I, I32 = C.c_void_p, C.c_int, C.c_int32
+    sig = {
+        "spork_page_bytes": ([P], C.c_size_t),
+        "spork_create": ([P, P, P, P], I),
+        "spork_destroy": ([P], I),
+        "spork_seq_create": ([P, I, P], I),
+        "spork_append": ([P, I, P, P, P, P, P], I),
+        "spork_fork": ([P, I, P, P, P], I),
+        "spork_release": ([P, I, P, P], I),
+        "spork_truncate": ([P, I, P, P, P], I),
+        "spork_decode_attn": ([P, I, P, P, P, P, P, P], I),
+        "spork_verify_attn": ([P, I, P, P, P, P, P, P, P], I),
+        "spork_decode_attn_host": ([P, I, P, P, P, P, P, P], I),
+        "spork_verify_attn_host": ([P, I, P, P, P, P, P, P, P], I),
+        "spork_export": ([P, I32, P, P], I),
+        "spork_export_refcounts": ([P, P], I),
+        "spork_read_kv": ([P, I32, I32, I32, P, P], I),
+        "spork_free_pages": ([P, P], I),
+        "spork_status": ([P], I),
+        "spork_last_plan": ([P, P], I),
+        "spork_last_launches": ([P], I),
+        "spork_strerror": ([I], C.c_char_p),
+    }
+    for name, (args, res) in sig.items():
+        f = getattr(lib, name)
+        f.argtypes = args
+        f.restype = res
+    _lib = lib
+    return lib
+
+
+class SporkError(RuntimeError):
+    def __init__(self, code: int):
+        msg = load().spork_strerror(code).decode()
+        super().__init__(f"spork error {code}: {msg}")
+        self.code = code
+
+
+def _i32(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32).reshape(-1))
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class Spork:
+    """One libspork handle plus the torch-allocated KV pools it works on."""
+
+    def __init__(self, dtype: str, Hq: int, Hkv: int, D: int, num_pages: int, max_seqs: int,
+                 max_pages_per_seq: int, scale: float, device: str = "cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libspork needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.lib = load()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.dtype, self.Hq, self.Hkv, self.D = dtype, Hq, Hkv, D
+        self.num_pages, self.max_seqs, self.max_pages_per_seq = num_pages, max_seqs, max_pages_per_seq
+        self.scale = float(scale)
+        self.ps = PAGE_SIZE
+        self.np_dtype = np.float32 if dtype == "f32" else np.uint16
+        self.torch_dtype = torch.float32 if dtype == "f32" else torch.bfloat16
+        self.cfg = SporkConfig({"f32": F32, "bf16": BF16}[dtype], Hq, Hkv, D, PAGE_SIZE, num_pages,
+                               max_seqs, max_pages_per_seq, self.scale)
+        self.page_bytes = int(self.lib.spork_page_bytes(C.byref(self.cfg)))
+        # caller-owned pools: raw bytes (torch.empty: contents arbitrary on purpose)
+        self.k_pool = torch.empty(num_pages * self.page_bytes, dtype=torch.uint8, device=self.device)
+        self.v_pool = torch.empty(num_pages * self.page_bytes, dtype=torch.uint8, device=self.device)
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+        h = C.c_void_p()
+        rc = self.lib.spork_create(C.byref(self.cfg), self.k_pool.data_ptr(), self.v_pool.data_ptr(),
+                                   C.byref(h))
+        if rc != OK:
+            raise SporkError(rc)
+        self._h = h
+
+    # ---- lifetime -------------------------------------------------------------
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.spork_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def _st(self):
+        return C.c_void_p(self.stream.cuda_stream)
+
+    def _enter(self):
+        """our stream waits for work queued on torch's current stream (caller-made inputs)"""
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)
+
+    def _leave(self):
+        """torch's current stream waits for ours, so results are safe to use there"""
+        cur = self.torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
+    @staticmethod
+    def _chk(rc: int, check: bool = True) -> int:
+        if rc != OK and check:
+            raise SporkError(rc)
+        return rc
+
+    def _dev(self, a: np.ndarray):
+        """numpy storage array (float32 / bf16 bit patterns) -> device tensor on our stream."""
+        t = self.torch.from_numpy(np.ascontiguousarray(a))
+        with self.torch.cuda.stream(self.stream):
+            return t.to(self.device, non_blocking=False)
+
+    # ---- state calls ----------------------------------------------------------
+    def seq_create(self, n: int) -> np.ndarray:
+        ids = np.zeros(n, np.int32)
+        self._chk(self.lib.spork_seq_create(self._h, n, _p(ids)))
+        return ids
+
+    def append(self, seq_ids, n_tokens, k, v, check: bool = True) -> int:
+        """k, v: numpy storage arrays or device tensors, [sum n_tokens][Hkv][D]."""
+        s, nt = _i32(seq_ids), _i32(n_tokens)
+        kd = k if hasattr(k, "data_ptr") else self._dev(np.asarray(k, dtype=self.np_dtype))
+        vd = v if hasattr(v, "data_ptr") else self._dev(np.asarray(v, dtype=self.np_dtype))
+        total = int(nt[nt > 0].sum()) if len(nt) else 0
+        assert kd.numel() * kd.element_size() == total * self.Hkv * self.D * (4 if self.dtype == "f32" else 2)
+        self._enter()
+        rc = self.lib.spork_append(self._h, len(s), _p(s), _p(nt), kd.data_ptr(), vd.data_ptr(), self._st)
+        self._keep = (kd, vd)   # stream-ordered use: keep alive until the next call
+        return self._chk(rc, check)
+
+    def fork(self, parents, check: bool = True):
+        p = _i32(parents)
+        ch = np.full(len(p), -1, np.int32)
+        rc = self._chk(self.lib.spork_fork(self._h, len(p), _p(p), _p(ch), self._st), check)
+        return ch if check else (rc, ch)
+
+    def release(self, seq_ids, check: bool = True) -> int:
+        s = _i32(seq_ids)
+        return self._chk(self.lib.spork_release(self._h, len(s), _p(s), self._st), check)
+
+    def truncate(self, seq_ids, new_len, check: bool = True) -> int:
+        s, nl = _i32(seq_ids), _i32(new_len)
+        return self._chk(self.lib.spork_truncate(self._h, len(s), _p(s), _p(nl), self._st), check)
+
+    # ---- attention ------------------------------------------------------------
+    def decode_attn(self, group_indptr, seq_ids, q, out=None, lse=None, check: bool = True):
+        """q: device tensor [n_seq][Hq][D] in the storage dtype (or numpy storage array).
+        Returns device fp32 tensors (out [n_seq][Hq][D], lse [n_seq][Hq])."""
+        torch = self.torch
+        gi, s = _i32(group_indptr), _i32(seq_ids)
+        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.np_dtype))
+        n = len(s)
+        if out is None:
+            out = torch.empty((n, self.Hq, self.D), dtype=torch.float32, device=self.device)
+        if lse is None:
+            lse = torch.empty((n, self.Hq), dtype=torch.float32, device=self.device)
+        self._enter()
+        rc = self.lib.spork_decode_attn(self._h, len(gi) - 1, _p(gi), _p(s), qd.data_ptr(),
+                                        out.data_ptr(), lse.data_ptr(), self._st)
+        self._leave()
+        self._keep = (qd,)
+        self._chk(rc, check)
+        return (out, lse) if check else (rc, out, lse)
+
+    def verify_attn(self, group_indptr, seq_ids, q_indptr, q, out=None, lse=None, check: bool = True):
+        torch = self.torch
+        gi, s, qi = _i32(group_indptr), _i32(seq_ids), _i32(q_indptr)
+        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.np_dtype))
+        rows = int(qi[-1]) if len(qi) else 0
+        if out is None:
+            out = torch.empty((rows, self.Hq, self.D), dtype=torch.float32, device=self.device)
+        if lse is None:
+            lse = torch.empty((rows, self.Hq), dtype=torch.float32, device=self.device)
+        self._enter()
+        rc = self.lib.spork_verify_attn(self._h, len(gi) - 1, _p(gi), _p(s), _p(qi), qd.data_ptr(),
+                                        out.data_ptr(), lse.data_ptr(), self._st)
+        self._leave()
+        self._keep = (qd,)
+        self._chk(rc, check)
+        return (out, lse) if check else (rc, out, lse)
+
+    def decode_attn_host(self, group_indptr, seq_ids, q_host, out_host, lse_host):
+        """HOST (pinned) tensors in, HOST tensors out; copies run inside the call."""
+        gi, s = _i32(group_indptr), _i32(seq_ids)
+        self._chk(self.lib.spork_decode_attn_host(self._h, len(gi) - 1, _p(gi), _p(s), q_host.data_ptr(),
+                                                  out_host.data_ptr(), lse_host.data_ptr(), self._st))
+
+    def verify_attn_host(self, group_indptr, seq_ids, q_indptr, q_host, out_host, lse_host):
+        gi, s, qi = _i32(group_indptr), _i32(seq_ids), _i32(q_indptr)
+        self._chk(self.lib.spork_verify_attn_host(self._h, len(gi) - 1, _p(gi), _p(s), _p(qi),
+                                                  q_host.data_ptr(), out_host.data_ptr(),
+                                                  lse_host.data_ptr(), self._st))
+
+    # ---- export ---------------------------------------------------------------
+    def export(self, seq: int):
+        """(len, table[ceil(len/16)]) read from the device; len = -1 if the slot is not live."""
+        ln = np.zeros(1, np.int32)
+        tab = np.full(self.max_pages_per_seq, -1, np.int32)
+        self._chk(self.lib.spork_export(self._h, int(seq), _p(ln), _p(tab)))
+        L = int(ln[0])
+        return L, tab[:max(0, (L + self.ps - 1) // self.ps)].copy()
+
+    export_seq = export   # same name as the oracle's engine interface
+
+    def export_refcounts(self) -> np.ndarray:
+        out = np.zeros(self.num_pages, np.int32)
+        self._chk(self.lib.spork_export_refcounts(self._h, _p(out)))
+        return out
+
+    def read_kv(self, seq: int, t0: int, n: int):
+        k = np.zeros((n, self.Hkv, self.D), self.np_dtype)
+        v = np.zeros_like(k)
+        self._chk(self.lib.spork_read_kv(self._h, int(seq), int(t0), int(n), _p(k), _p(v)))
+        return k, v
+
+    def free_pages(self) -> int:
+        out = np.zeros(1, np.int32)
+        self._chk(self.lib.spork_free_pages(self._h, _p(out)))
+        return int(out[0])
+
+    def status(self) -> int:
+        return int(self.lib.spork_status(self._h))
+
+    def last_plan(self) -> dict:
+        info = PlanInfo()
+        self._chk(self.lib.spork_last_plan(self._h, C.byref(info)))
+        return info.as_dict()
+
+    def last_launches(self) -> int:
+        return int(self.lib.spork_last_launches(self._h))
+
+    def synchronize(self):
+        self.stream.synchronize()

@@ -1,0 +1,570 @@
+// libspork: page allocator (lowest free id first), append, fork, release, truncate.
+//
+// Device state: refcount[NP] (0 <=> free, reading A-2), table[S][stride],
+// len[S], counters[0] = free pages.  The host mirrors only lengths and slot
+// occupancy (to size grids and validate arguments); tables and refcounts are
+// produced by these kernels alone.
+#include <string.h>
+
+#include <algorithm>
+
+#include "spork_internal.h"
+
+using namespace spork;
+
+namespace {
+
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_PER_THREAD = 16;
+constexpr int SCAN_BLOCK = SCAN_THREADS * SCAN_PER_THREAD;  // 4096 pages per block
+
+__device__ __forceinline__ int block_exclusive_scan(int v, int *total, int *smem /*[33]*/) {
+    // 256 threads: warp scan + scan of the 8 warp totals
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) smem[w] = x;
+    __syncthreads();
+    if (w == 0) {
+        int t = lane < (int)(blockDim.x >> 5) ? smem[lane] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, t, o);
+            if (lane >= o) t += y;
+        }
+        smem[lane] = t;  // inclusive warp totals
+    }
+    __syncthreads();
+    int base = w ? smem[w - 1] : 0;
+    *total = smem[(blockDim.x >> 5) - 1];
+    return base + x - v;
+}
+
+// pass 1: number of free pages in each 4096-page block
+__global__ void __launch_bounds__(SCAN_THREADS) free_count_kernel(const int32_t *__restrict__ refcount,
+                                                                  int num_pages,
+                                                                  int32_t *__restrict__ block_counts) {
+    __shared__ int sm[33];
+    int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_PER_THREAD;
+    int cnt = 0;
+    if (base + SCAN_PER_THREAD <= num_pages) {
+        const int4 *p = reinterpret_cast<const int4 *>(refcount + base);
+#pragma unroll
+        for (int i = 0; i < SCAN_PER_THREAD / 4; ++i) {
+            int4 v = p[i];
+            cnt += (v.x == 0) + (v.y == 0) + (v.z == 0) + (v.w == 0);
+        }
+    } else {
+        for (int i = 0; i < SCAN_PER_THREAD; ++i)
+            if (base + i < num_pages) cnt += refcount[base + i] == 0;
+    }
+    int total;
+    block_exclusive_scan(cnt, &total, sm);
+    if (threadIdx.x == 0) block_counts[blockIdx.x] = total;
+}
+
+// pass 2: exclusive scan of the block counts (single block, any length)
+__global__ void __launch_bounds__(SCAN_THREADS) scan_blocks_kernel(int32_t *block_counts, int n) {
+    __shared__ int sm[33];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int b = 0; b < n; b += SCAN_THREADS) {
+        int i = b + threadIdx.x;
+        int v = i < n ? block_counts[i] : 0;
+        int total;
+        int ex = block_exclusive_scan(v, &total, sm);
+        int c0 = carry;
+        if (i < n) block_counts[i] = c0 + ex;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = c0 + total;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) block_counts[n] = carry;  // total free pages
+}
+
+// pass 3: write the ids of the `need` lowest free pages, ascending
+__global__ void __launch_bounds__(SCAN_THREADS) free_compact_kernel(
+    const int32_t *__restrict__ refcount, int num_pages, const int32_t *__restrict__ block_offsets,
+    int need, int32_t *__restrict__ free_list) {
+    __shared__ int sm[33];
+    int boff = block_offsets[blockIdx.x];
+    if (boff >= need) return;
+    int base = blockIdx.x * SCAN_BLOCK + threadIdx.x * SCAN_PER_THREAD;
+    unsigned mask = 0;
+    if (base + SCAN_PER_THREAD <= num_pages) {
+        const int4 *p = reinterpret_cast<const int4 *>(refcount + base);
+#pragma unroll
+        for (int i = 0; i < SCAN_PER_THREAD / 4; ++i) {
+            int4 v = p[i];
+            mask |= (unsigned)(v.x == 0) << (4 * i) | (unsigned)(v.y == 0) << (4 * i + 1) |
+                    (unsigned)(v.z == 0) << (4 * i + 2) | (unsigned)(v.w == 0) << (4 * i + 3);
+        }
+    } else {
+        for (int i = 0; i < SCAN_PER_THREAD; ++i)
+            if (base + i < num_pages && refcount[base + i] == 0) mask |= 1u << i;
+    }
+    int total;
+    int rank = boff + block_exclusive_scan(__popc(mask), &total, sm);
+    while (mask && rank < need) {
+        int i = __ffs(mask) - 1;
+        mask &= mask - 1;
+        free_list[rank++] = base + i;
+    }
+}
+
+// ---- append ----------------------------------------------------------------
+struct AppendDesc {
+    int32_t seq, old_len, n_tok, tok_off;
+    int32_t free_off;   // index into free_list of this request's first new page
+    int32_t n_new;      // pages this request allocates
+    int32_t final_len;  // >= 0: this request writes len[seq] (last request of the sequence)
+    int32_t pad;
+};
+
+__global__ void append_assign_kernel(const AppendDesc *__restrict__ descs, int n,
+                                     const int32_t *__restrict__ free_list, int32_t *refcount,
+                                     int32_t *table, int table_stride, int32_t *len, int32_t *counters,
+                                     int need) {
+    int i = blockIdx.x;
+    AppendDesc d = descs[i];
+    int first_new = pages_of(d.old_len);
+    for (int j = threadIdx.x; j < d.n_new; j += blockDim.x) {
+        int p = free_list[d.free_off + j];
+        table[(size_t)d.seq * table_stride + first_new + j] = p;
+        refcount[p] = 1;
+    }
+    if (threadIdx.x == 0) {
+        if (d.final_len >= 0) len[d.seq] = d.final_len;
+        if (i == 0 && need) atomicSub(&counters[0], need);
+    }
+}
+
+// one thread per 16-byte chunk of one (token, kv head) row; K and V together
+__global__ void __launch_bounds__(256) append_copy_kernel(
+    const AppendDesc *__restrict__ descs, int n, const uint4 *__restrict__ k_src,
+    const uint4 *__restrict__ v_src, uint8_t *__restrict__ k_pool, uint8_t *__restrict__ v_pool,
+    const int32_t *__restrict__ table, int table_stride, int Hkv, int chunks_per_row /* D*elt/16 */,
+    int swizzled, size_t head_block, size_t total_units) {
+    for (size_t u = blockIdx.x * (size_t)blockDim.x + threadIdx.x; u < total_units;
+         u += (size_t)gridDim.x * blockDim.x) {
+        int c = (int)(u % chunks_per_row);
+        int h = (int)((u / chunks_per_row) % Hkv);
+        int tok = (int)(u / ((size_t)chunks_per_row * Hkv));
+        // request containing flat token `tok`: last i with tok_off <= tok
+        int lo = 0, hi = n - 1;
+        while (lo < hi) {
+            int mid = (lo + hi + 1) >> 1;
+            if (descs[mid].tok_off <= tok) lo = mid; else hi = mid - 1;
+        }
+        // requests with n_tok == 0 share tok_off with their successor: the search lands on the last
+        // of them, which is the one that owns the token
+        AppendDesc d = descs[lo];
+        int pos = d.old_len + (tok - d.tok_off);
+        int page = table[(size_t)d.seq * table_stride + pos / PS];
+        int r = pos % PS;
+        size_t off;
+        if (swizzled) {
+            int half = c >> 3, cc = c & 7;
+            off = (size_t)half * (PS * 128) + (size_t)r * 128 + (size_t)((cc ^ (r & 7)) << 4);
+        } else {
+            off = ((size_t)r * chunks_per_row + c) * 16;
+        }
+        size_t dst = ((size_t)page * Hkv + h) * head_block + off;
+        *reinterpret_cast<uint4 *>(k_pool + dst) = k_src[u];
+        *reinterpret_cast<uint4 *>(v_pool + dst) = v_src[u];
+    }
+}
+
+// ---- fork ------------------------------------------------------------------
+struct ForkDesc {
+    int32_t parent, child, len, tail_idx;  // tail_idx: index into free_list, or -1
+};
+struct ParentDesc {
+    int32_t parent, count, nf, pad;
+};
+
+// one block per fork: clone the table row (16-byte vectors), then duplicate the tail page
+__global__ void __launch_bounds__(256) fork_clone_kernel(
+    const ForkDesc *__restrict__ descs, const int32_t *__restrict__ free_list, int32_t *table,
+    int table_stride, int32_t *len, int32_t *refcount, uint8_t *k_pool, uint8_t *v_pool,
+    size_t page_bytes, int32_t *counters, int need) {
+    __shared__ int s_tail;
+    ForkDesc d = descs[blockIdx.x];
+    int nf = d.len / PS;
+    int tail_page = d.tail_idx >= 0 ? free_list[d.tail_idx] : -1;
+    const int4 *src = reinterpret_cast<const int4 *>(table + (size_t)d.parent * table_stride);
+    int4 *dst = reinterpret_cast<int4 *>(table + (size_t)d.child * table_stride);
+    int n4 = (nf + 1 + 3) / 4;                       // covers entries [0, nf]
+    if (n4 * 4 > table_stride) n4 = table_stride / 4;
+    int parent_tail = -1;
+    for (int j = threadIdx.x; j < n4; j += blockDim.x) {
+        int4 v = src[j];
+        int e[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            int idx = j * 4 + q;
+            if (idx == nf) { parent_tail = e[q]; e[q] = tail_page; }
+            else if (idx > nf) e[q] = -1;
+        }
+        dst[j] = make_int4(e[0], e[1], e[2], e[3]);
+    }
+    if (threadIdx.x == 0) {
+        len[d.child] = d.len;
+        if (tail_page >= 0) refcount[tail_page] = 1;
+        if (blockIdx.x == 0 && need) atomicSub(&counters[0], need);
+    }
+    if (tail_page < 0) return;
+    // the thread that saw entry nf broadcasts the parent's tail page id
+    if (parent_tail >= 0) s_tail = parent_tail;
+    __syncthreads();
+    size_t n16 = page_bytes / 16;
+    const uint4 *ks = reinterpret_cast<const uint4 *>(k_pool + (size_t)s_tail * page_bytes);
+    const uint4 *vs = reinterpret_cast<const uint4 *>(v_pool + (size_t)s_tail * page_bytes);
+    uint4 *kd = reinterpret_cast<uint4 *>(k_pool + (size_t)tail_page * page_bytes);
+    uint4 *vd = reinterpret_cast<uint4 *>(v_pool + (size_t)tail_page * page_bytes);
+    for (size_t j = threadIdx.x; j < n16; j += blockDim.x) {
+        kd[j] = ks[j];
+        vd[j] = vs[j];
+    }
+}
+
+// one block per (distinct parent, 1024-entry chunk): refcount[page] += number of forks of that parent
+__global__ void __launch_bounds__(256) fork_refcount_kernel(const ParentDesc *__restrict__ pd,
+                                                            const int32_t *__restrict__ table,
+                                                            int table_stride, int32_t *refcount) {
+    ParentDesc d = pd[blockIdx.y];
+    const int32_t *row = table + (size_t)d.parent * table_stride;
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < d.nf; j += gridDim.x * blockDim.x)
+        atomicAdd(&refcount[row[j]], d.count);
+}
+
+// ---- release / truncate ------------------------------------------------------
+struct DropDesc {
+    int32_t seq, keep_pages, n_pages, new_len;
+};
+
+// one block per sequence: drop one reference from pages [keep_pages, n_pages)
+__global__ void __launch_bounds__(256) drop_pages_kernel(const DropDesc *__restrict__ descs,
+                                                         int32_t *table, int table_stride,
+                                                         int32_t *len, int32_t *refcount,
+                                                         int32_t *counters) {
+    __shared__ int s_freed;
+    DropDesc d = descs[blockIdx.x];
+    if (threadIdx.x == 0) s_freed = 0;
+    __syncthreads();
+    int32_t *row = table + (size_t)d.seq * table_stride;
+    int freed = 0;
+    for (int j = d.keep_pages + threadIdx.x; j < d.n_pages; j += blockDim.x) {
+        int p = row[j];
+        row[j] = -1;
+        if (p < 0) { atomicExch(&counters[1], 1); continue; }   // consistency check
+        int old = atomicSub(&refcount[p], 1);
+        if (old == 1) ++freed;
+        if (old <= 0) atomicExch(&counters[1], 2);
+    }
+    for (int o = 16; o; o >>= 1) freed += __shfl_down_sync(0xffffffffu, freed, o);
+    if ((threadIdx.x & 31) == 0 && freed) atomicAdd(&s_freed, freed);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_freed) atomicAdd(&counters[0], s_freed);
+        len[d.seq] = d.new_len;
+    }
+}
+
+__global__ void check_shared_kernel(const DropDesc *__restrict__ descs, int n,
+                                    const int32_t *__restrict__ table, int table_stride,
+                                    const int32_t *__restrict__ refcount, int32_t *flag) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        DropDesc d = descs[i];
+        if (d.new_len % PS) {
+            int p = table[(size_t)d.seq * table_stride + d.new_len / PS];
+            if (p < 0 || refcount[p] > 1) *flag = 1;
+        }
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------
+namespace spork {
+
+int launch_free_scan(spork_ctx *c, int need, cudaStream_t st) {
+    if (need <= 0) return SPORK_OK;
+    if ((size_t)need > c->free_list_cap) {
+        SPORK_CUDA(cudaStreamSynchronize(st));
+        cudaFree(c->d_free_list);
+        c->d_free_list = nullptr;
+        c->free_list_cap = (size_t)need * 2;
+        SPORK_CUDA(cudaMalloc(&c->d_free_list, c->free_list_cap * 4));
+    }
+    int nb = ceil_div(c->cfg.num_pages, SCAN_BLOCK);
+    free_count_kernel<<<nb, SCAN_THREADS, 0, st>>>(c->d_refcount, c->cfg.num_pages, c->d_scan);
+    scan_blocks_kernel<<<1, SCAN_THREADS, 0, st>>>(c->d_scan, nb);
+    free_compact_kernel<<<nb, SCAN_THREADS, 0, st>>>(c->d_refcount, c->cfg.num_pages, c->d_scan, need,
+                                                     c->d_free_list);
+    c->last_launches += 3;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
+int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st) {
+    if (need <= c->free_lb) return SPORK_OK;
+    // the lower bound cannot prove it: read the exact device count (documented sync)
+    SPORK_CUDA(cudaStreamSynchronize(st));
+    int32_t f = 0;
+    SPORK_CUDA(cudaMemcpy(&f, c->d_counters, 4, cudaMemcpyDeviceToHost));
+    c->free_lb = f;
+    return need <= c->free_lb ? SPORK_OK : SPORK_ERR_OOM;
+}
+
+}  // namespace spork
+
+// ---------------------------------------------------------------------------
+extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const int32_t *n_tokens,
+                            const void *k_src, const void *v_src, void *stream) {
+    if (!c || n < 0 || (n > 0 && (!seq_ids || !n_tokens))) return SPORK_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    // validate the whole batch against evolving lengths; nothing changes on failure
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        if (s >= 0 && s < c->cfg.max_seqs && c->h_live[s]) c->h_scratch[s] = c->h_len[s];
+    }
+    int64_t need = 0, total = 0;
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        if (s < 0 || s >= c->cfg.max_seqs || !c->h_live[s] || n_tokens[i] < 0)
+            return SPORK_ERR_INVALID_SEQ;
+        int64_t nl = (int64_t)c->h_scratch[s] + n_tokens[i];
+        if ((nl + PS - 1) / PS > c->cfg.max_pages_per_seq) return SPORK_ERR_TOO_LONG;
+        need += pages_of((int)nl) - pages_of(c->h_scratch[s]);
+        c->h_scratch[s] = (int)nl;
+        total += n_tokens[i];
+    }
+    if (total > 0 && (!k_src || !v_src)) return SPORK_ERR_INVALID;
+    if (total >= (int64_t)1 << 31) return SPORK_ERR_INVALID;
+    int rc = ensure_pages(c, need, st);
+    if (rc != SPORK_OK) return rc;
+
+    StageSlot *slot;
+    rc = stage_acquire(c, sizeof(AppendDesc) * (size_t)n, &slot);
+    if (rc != SPORK_OK) return rc;
+    AppendDesc *d = (AppendDesc *)slot->h;
+    for (int i = 0; i < n; ++i) c->h_scratch[seq_ids[i]] = -1;  // marks "last request not yet seen"
+    int tok = 0, foff = 0;
+    // final_len is written by the LAST request of each sequence: walk backwards to mark it
+    for (int i = n - 1; i >= 0; --i) {
+        int s = seq_ids[i];
+        d[i].final_len = c->h_scratch[s] == -1 ? 0 : -1;  // placeholder 0 = "is last"
+        c->h_scratch[s] = 0;
+    }
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        int ol = c->h_len[s], nl = ol + n_tokens[i];
+        d[i].seq = s;
+        d[i].old_len = ol;
+        d[i].n_tok = n_tokens[i];
+        d[i].tok_off = tok;
+        d[i].free_off = foff;
+        d[i].n_new = pages_of(nl) - pages_of(ol);
+        d[i].final_len = d[i].final_len == 0 ? nl : -1;
+        d[i].pad = 0;
+        tok += n_tokens[i];
+        foff += d[i].n_new;
+        c->h_len[s] = nl;
+    }
+    rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
+    if (rc != SPORK_OK) return rc;
+    rc = launch_free_scan(c, (int)need, st);
+    if (rc != SPORK_OK) return rc;
+    append_assign_kernel<<<n, 128, 0, st>>>((const AppendDesc *)slot->d, n, c->d_free_list,
+                                            c->d_refcount, c->d_table, c->table_stride, c->d_len,
+                                            c->d_counters, (int)need);
+    c->last_launches++;
+    if (total > 0) {
+        int cpr = c->cfg.head_dim * c->elt / 16;
+        size_t units = (size_t)total * c->cfg.num_kv_heads * cpr;
+        int blocks = (int)std::min<size_t>((units + 255) / 256, (size_t)c->num_sms * 16);
+        append_copy_kernel<<<blocks, 256, 0, st>>>(
+            (const AppendDesc *)slot->d, n, (const uint4 *)k_src, (const uint4 *)v_src,
+            (uint8_t *)c->k_pool, (uint8_t *)c->v_pool, c->d_table, c->table_stride,
+            c->cfg.num_kv_heads, cpr, c->swizzled, c->head_block, units);
+        c->last_launches++;
+    }
+    SPORK_CUDA(cudaGetLastError());
+    c->free_lb -= need;
+    c->len_epoch++;
+    return stage_done(c, slot, st);
+}
+
+extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_t *child_ids_out,
+                          void *stream) {
+    if (!c || n < 0 || (n > 0 && (!parent_ids || !child_ids_out))) return SPORK_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    int64_t need = 0;
+    for (int i = 0; i < n; ++i) {
+        int p = parent_ids[i];
+        if (p < 0 || p >= c->cfg.max_seqs || !c->h_live[p]) return SPORK_ERR_INVALID_SEQ;
+        need += (c->h_len[p] % PS) != 0;
+    }
+    if (c->cfg.max_seqs - c->n_live < n) return SPORK_ERR_NO_SLOT;
+    int rc = ensure_pages(c, need, st);
+    if (rc != SPORK_OK) return rc;
+
+    size_t bytes = sizeof(ForkDesc) * (size_t)n + sizeof(ParentDesc) * (size_t)n;
+    StageSlot *slot;
+    rc = stage_acquire(c, bytes, &slot);
+    if (rc != SPORK_OK) return rc;
+    ForkDesc *fd = (ForkDesc *)slot->h;
+    ParentDesc *pd = (ParentDesc *)(fd + n);
+    // count forks per distinct parent (h_scratch as a per-slot counter)
+    for (int i = 0; i < n; ++i) c->h_scratch[parent_ids[i]] = 0;
+    int n_par = 0, max_nf = 0;
+    for (int i = 0; i < n; ++i) {
+        int p = parent_ids[i];
+        if (c->h_scratch[p]++ == 0) {
+            pd[n_par].parent = p;
+            pd[n_par].nf = c->h_len[p] / PS;
+            pd[n_par].pad = 0;
+            max_nf = std::max(max_nf, pd[n_par].nf);
+            ++n_par;
+        }
+    }
+    for (int j = 0; j < n_par; ++j) pd[j].count = c->h_scratch[pd[j].parent];
+    // children: lowest free slots in request order
+    int tail = 0;
+    for (int i = 0, s = 0; i < n; ++s) {
+        if (c->h_live[s]) continue;
+        int p = parent_ids[i], L = c->h_len[p];
+        c->h_live[s] = 1;
+        c->h_len[s] = L;
+        c->h_shared_upto[s] = L / PS;
+        c->h_shared_upto[p] = std::max(c->h_shared_upto[p], L / PS);
+        fd[i].parent = p;
+        fd[i].child = s;
+        fd[i].len = L;
+        fd[i].tail_idx = (L % PS) ? tail++ : -1;
+        child_ids_out[i] = s;
+        ++i;
+    }
+    c->n_live += n;
+    rc = stage_commit(c, slot, bytes, st);
+    if (rc != SPORK_OK) return rc;
+    rc = launch_free_scan(c, (int)need, st);
+    if (rc != SPORK_OK) return rc;
+    if (max_nf > 0) {
+        dim3 grid(std::max(1, std::min(ceil_div(max_nf, 1024), 64)), n_par);
+        fork_refcount_kernel<<<grid, 256, 0, st>>>((const ParentDesc *)((ForkDesc *)slot->d + n),
+                                                   c->d_table, c->table_stride, c->d_refcount);
+        c->last_launches++;
+    }
+    fork_clone_kernel<<<n, 256, 0, st>>>((const ForkDesc *)slot->d, c->d_free_list, c->d_table,
+                                         c->table_stride, c->d_len, c->d_refcount,
+                                         (uint8_t *)c->k_pool, (uint8_t *)c->v_pool, c->page_bytes,
+                                         c->d_counters, (int)need);
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    c->free_lb -= need;
+    c->structure_epoch++;
+    c->len_epoch++;
+    return stage_done(c, slot, st);
+}
+
+static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_t *new_len,
+                       cudaStream_t st) {
+    // new_len == nullptr: release.  Errors are reported for the first offending request in array
+    // order; a possibly-shared kept tail page BEFORE that request is resolved on the device first.
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        if (s >= 0 && s < c->cfg.max_seqs) c->h_scratch[s] = 0;
+    }
+    int n_ok = n, host_err = SPORK_OK;
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        if (s < 0 || s >= c->cfg.max_seqs || !c->h_live[s] || c->h_scratch[s]++) {
+            host_err = SPORK_ERR_INVALID_SEQ;
+            n_ok = i;
+            break;
+        }
+        if (new_len && (new_len[i] < 0 || new_len[i] > c->h_len[s])) {
+            host_err = SPORK_ERR_INVALID;
+            n_ok = i;
+            break;
+        }
+    }
+    if (n_ok == 0) return host_err;
+    StageSlot *slot;
+    int rc = stage_acquire(c, sizeof(DropDesc) * (size_t)n_ok, &slot);
+    if (rc != SPORK_OK) return rc;
+    DropDesc *d = (DropDesc *)slot->h;
+    bool need_check = false;
+    for (int i = 0; i < n_ok; ++i) {
+        int s = seq_ids[i];
+        d[i].seq = s;
+        d[i].n_pages = pages_of(c->h_len[s]);
+        d[i].new_len = new_len ? new_len[i] : 0;
+        d[i].keep_pages = new_len ? pages_of(new_len[i]) : 0;
+        // a partially filled kept tail page can only be shared below h_shared_upto
+        if (new_len && (new_len[i] % PS) && new_len[i] / PS < c->h_shared_upto[s]) need_check = true;
+    }
+    if (host_err != SPORK_OK && !need_check) return host_err;
+    rc = stage_commit(c, slot, sizeof(DropDesc) * (size_t)n_ok, st);
+    if (rc != SPORK_OK) return rc;
+    if (need_check) {
+        // exact answer needs the device refcounts: check, then read the flag (documented sync)
+        SPORK_CUDA(cudaMemsetAsync(c->d_counters + 2, 0, 4, st));
+        check_shared_kernel<<<ceil_div(n_ok, 256), 256, 0, st>>>((const DropDesc *)slot->d, n_ok,
+                                                                 c->d_table, c->table_stride,
+                                                                 c->d_refcount, c->d_counters + 2);
+        c->last_launches++;
+        int32_t flag = 0;
+        SPORK_CUDA(cudaMemcpyAsync(&flag, c->d_counters + 2, 4, cudaMemcpyDeviceToHost, st));
+        SPORK_CUDA(cudaStreamSynchronize(st));
+        if (flag || host_err != SPORK_OK) {
+            stage_done(c, slot, st);
+            return flag ? SPORK_ERR_SHARED : host_err;
+        }
+    }
+    drop_pages_kernel<<<n, 256, 0, st>>>((const DropDesc *)slot->d, c->d_table, c->table_stride,
+                                         c->d_len, c->d_refcount, c->d_counters);
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    for (int i = 0; i < n; ++i) {
+        int s = seq_ids[i];
+        if (new_len) {
+            c->h_len[s] = new_len[i];
+            c->h_shared_upto[s] = std::min(c->h_shared_upto[s], pages_of(new_len[i]));
+        } else {
+            c->h_len[s] = 0;
+            c->h_live[s] = 0;
+            c->h_shared_upto[s] = 0;
+        }
+    }
+    if (!new_len) c->n_live -= n;
+    c->structure_epoch++;
+    c->len_epoch++;
+    return stage_done(c, slot, st);
+}
+
+extern "C" int spork_release(spork_ctx *c, int n, const int32_t *seq_ids, void *stream) {
+    if (!c || n < 0 || (n > 0 && !seq_ids)) return SPORK_ERR_INVALID;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    return drop_common(c, n, seq_ids, nullptr, (cudaStream_t)stream);
+}
+
+extern "C" int spork_truncate(spork_ctx *c, int n, const int32_t *seq_ids, const int32_t *new_len,
+                              void *stream) {
+    if (!c || n < 0 || (n > 0 && (!seq_ids || !new_len))) return SPORK_ERR_INVALID;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    return drop_common(c, n, seq_ids, new_len, (cudaStream_t)stream);
+}

@@ -1,0 +1,236 @@
+// libspork: generic CUDA-core attention kernel (fp32 KV, or bf16 with D != 128)
+// and the LSE merge kernel shared by both attention paths.
+//
+// simt kernel: one CTA per work item, one warp per query row at a time.  A
+// lane owns one token for the score pass (full dot product, 16-byte loads) and
+// D/32 output dims for the value pass.  fp32 accumulation, accurate expf/logf:
+// this is the path that has to meet 1e-5 on fp32 KV (config 1), not a
+// bandwidth target.
+#include <math.h>
+
+#include "spork_internal.h"
+
+using namespace spork;
+
+namespace {
+
+constexpr int SIMT_WARPS = 4;
+
+__device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
+__device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xffff0000u); }
+
+// byte offset of 16-byte chunk c of row r inside a (page, kv head) block
+__device__ __forceinline__ int chunk_off(int swizzled, int chunks_per_row, int r, int c) {
+    if (swizzled) return (c >> 3) * (PS * 128) + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+    return (r * chunks_per_row + c) * 16;
+}
+
+template <typename T> struct Elt;
+template <> struct Elt<float> {
+    static constexpr int PER_CHUNK = 4;
+    static __device__ __forceinline__ void unpack(const uint4 &v, float *f) {
+        f[0] = __uint_as_float(v.x); f[1] = __uint_as_float(v.y);
+        f[2] = __uint_as_float(v.z); f[3] = __uint_as_float(v.w);
+    }
+    static __device__ __forceinline__ float load(const uint8_t *p) { return *reinterpret_cast<const float *>(p); }
+};
+template <> struct Elt<uint16_t> {
+    static constexpr int PER_CHUNK = 8;
+    static __device__ __forceinline__ void unpack(const uint4 &v, float *f) {
+        f[0] = bf16_lo(v.x); f[1] = bf16_hi(v.x); f[2] = bf16_lo(v.y); f[3] = bf16_hi(v.y);
+        f[4] = bf16_lo(v.z); f[5] = bf16_hi(v.z); f[6] = bf16_lo(v.w); f[7] = bf16_hi(v.w);
+    }
+    static __device__ __forceinline__ float load(const uint8_t *p) {
+        return __uint_as_float((uint32_t)(*reinterpret_cast<const uint16_t *>(p)) << 16);
+    }
+};
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+template <typename T, int DMAX>
+__global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
+    const WorkItem *__restrict__ items, const T *__restrict__ q, const uint8_t *__restrict__ k_pool,
+    const uint8_t *__restrict__ v_pool, const int32_t *__restrict__ table, int table_stride, int Hq,
+    int Hkv, int G, int D, int swizzled, float scale, float *__restrict__ ws_o,
+    float *__restrict__ ws_lse) {
+    __shared__ float qs[SIMT_WARPS][DMAX];
+    const WorkItem it = items[blockIdx.x];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    constexpr int E = Elt<T>::PER_CHUNK;
+    const int cpr = D / E;                       // 16-byte chunks per row
+    const size_t head_block = (size_t)PS * D * sizeof(T);
+    const int32_t *row_tab = table + (size_t)it.table_seq * table_stride;
+    constexpr int NACC = DMAX / 32;
+
+    for (int r = warp; r < it.nrows; r += SIMT_WARPS) {
+        const int lr = it.rb0 + r;
+        const int qrow = it.qrow0 + lr / G, h = it.kvh * G + lr % G;
+        const int lim = it.lim0 + lr / G;
+        __syncwarp();
+        for (int d = lane; d < D; d += 32)
+            qs[warp][d] = Elt<T>::load(reinterpret_cast<const uint8_t *>(q + ((size_t)qrow * Hq + h) * D + d));
+        __syncwarp();
+        float m = -INFINITY, l = 0.f, acc[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
+
+        for (int tb = it.tok0; tb < it.tok1; tb += 32) {
+            const int t = tb + lane;
+            const bool valid = t < it.tok1 && t <= lim;
+            float s = -INFINITY;
+            size_t blk = 0;
+            if (valid) {
+                blk = ((size_t)row_tab[t / PS] * Hkv + it.kvh) * head_block;
+                const uint8_t *kp = k_pool + blk;
+                float dot = 0.f;
+                for (int c = 0; c < cpr; ++c) {
+                    uint4 v = *reinterpret_cast<const uint4 *>(kp + chunk_off(swizzled, cpr, t % PS, c));
+                    float f[E];
+                    Elt<T>::unpack(v, f);
+#pragma unroll
+                    for (int e = 0; e < E; ++e) dot = fmaf(qs[warp][c * E + e], f[e], dot);
+                }
+                s = dot * scale;
+            }
+            const float m_new = fmaxf(m, warp_max(s));
+            if (m_new == -INFINITY) continue;   // nothing visible yet (warp-uniform)
+            const float alpha = expf(m - m_new);   // m = -inf -> 0
+            const float p = valid ? expf(s - m_new) : 0.f;
+            l = l * alpha + warp_sum(p);
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) acc[i] *= alpha;
+            m = m_new;
+            const int nt = min(32, it.tok1 - tb);
+            for (int tt = 0; tt < nt; ++tt) {
+                const float pt = __shfl_sync(0xffffffffu, p, tt);
+                const unsigned long long b = __shfl_sync(0xffffffffu, (unsigned long long)blk, tt);
+                if (pt == 0.f) continue;        // warp-uniform; also keeps 0 * garbage out
+                const uint8_t *vp = v_pool + b;
+                const int rr = (tb + tt) % PS;
+#pragma unroll
+                for (int i = 0; i < NACC; ++i) {
+                    int d = lane + 32 * i;
+                    if (d < D) {
+                        int off = chunk_off(swizzled, cpr, rr, d / E) + (d % E) * (int)sizeof(T);
+                        acc[i] = fmaf(pt, Elt<T>::load(vp + off), acc[i]);
+                    }
+                }
+            }
+        }
+        const size_t prow = (size_t)it.part_base + r;
+        const float inv = l > 0.f ? 1.f / l : 0.f;
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) {
+            int d = lane + 32 * i;
+            if (d < D) ws_o[prow * D + d] = acc[i] * inv;
+        }
+        if (lane == 0) ws_lse[prow] = l > 0.f ? m + logf(l) : -INFINITY;
+    }
+}
+
+// one warp per (q row, q head): LSE-weighted combination of that row's partials
+//   M = max lse_s, w_s = exp(lse_s - M), out = sum w_s o_s / sum w_s, lse = M + ln sum w_s
+// an empty partial has lse = -inf and weight 0; no partial at all: out = 0, lse = -inf
+__global__ void __launch_bounds__(256) merge_kernel(const QRowDesc *__restrict__ qd, int n_qrows, int Hq,
+                                                    int G, int D, const float *__restrict__ ws_o,
+                                                    const float *__restrict__ ws_lse,
+                                                    float *__restrict__ out, float *__restrict__ lse) {
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n_qrows * Hq) return;
+    const int qrow = w / Hq, h = w % Hq, kvh = h / G, j = h % G;
+    const QRowDesc d = qd[qrow];
+    const int pre0 = d.pre_base + kvh * d.pre_nq * G + d.pre_qi * G + j;
+    const int suf0 = d.suf_base + kvh * d.suf_nq * G + d.suf_qi * G + j;
+    const int n = d.pre_nsplit + d.suf_nsplit;
+    auto part = [&](int s) -> size_t {
+        return s < d.pre_nsplit ? (size_t)pre0 + (size_t)s * d.pre_stride
+                                : (size_t)suf0 + (size_t)(s - d.pre_nsplit) * d.suf_stride;
+    };
+    float M = -INFINITY;
+    for (int s = lane; s < n; s += 32) M = fmaxf(M, ws_lse[part(s)]);
+    M = warp_max(M);
+    float *o = out + (size_t)w * D;
+    if (M == -INFINITY) {
+        for (int dd = lane; dd < D; dd += 32) o[dd] = 0.f;
+        if (lane == 0) lse[w] = -INFINITY;
+        return;
+    }
+    float acc[8], W = 0.f;   // D <= 256
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] = 0.f;
+    for (int s = 0; s < n; ++s) {
+        const size_t p = part(s);
+        const float ws = expf(ws_lse[p] - M);
+        if (ws == 0.f) continue;
+        W += ws;
+        const float *po = ws_o + p * D;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            int dd = lane + 32 * i;
+            if (dd < D) acc[i] = fmaf(ws, po[dd], acc[i]);
+        }
+    }
+    const float inv = 1.f / W;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        int dd = lane + 32 * i;
+        if (dd < D) o[dd] = acc[i] * inv;
+    }
+    if (lane == 0) lse[w] = M + logf(W);
+}
+
+}  // namespace
+
+namespace spork {
+
+int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st) {
+    const Plan &P = c->plan;
+    if (P.n_items == 0) return SPORK_OK;
+    const WorkItem *items = (const WorkItem *)P.items.p;
+    float *wo = (float *)c->ws_o.p, *wl = (float *)c->ws_lse.p;
+    const uint8_t *kp = (const uint8_t *)c->k_pool, *vp = (const uint8_t *)c->v_pool;
+    const spork_config &f = c->cfg;
+    dim3 grid(P.n_items), block(SIMT_WARPS * 32);
+#define SPORK_SIMT(T, DMAX)                                                                        \
+    attn_simt_kernel<T, DMAX><<<grid, block, 0, st>>>(items, (const T *)q, kp, vp, c->d_table,     \
+                                                      c->table_stride, f.num_q_heads,              \
+                                                      f.num_kv_heads, c->G, f.head_dim,            \
+                                                      c->swizzled, f.scale, wo, wl)
+    if (f.dtype == SPORK_F32) {
+        if (f.head_dim <= 64) SPORK_SIMT(float, 64);
+        else if (f.head_dim <= 128) SPORK_SIMT(float, 128);
+        else SPORK_SIMT(float, 256);
+    } else {
+        if (f.head_dim <= 64) SPORK_SIMT(uint16_t, 64);
+        else if (f.head_dim <= 128) SPORK_SIMT(uint16_t, 128);
+        else SPORK_SIMT(uint16_t, 256);
+    }
+#undef SPORK_SIMT
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
+int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
+    const Plan &P = c->plan;
+    if (P.n_qrows == 0) return SPORK_OK;
+    const int warps = P.n_qrows * c->cfg.num_q_heads;
+    merge_kernel<<<ceil_div(warps, 8), 256, 0, st>>>((const QRowDesc *)P.qdesc.p, P.n_qrows,
+                                                     c->cfg.num_q_heads, c->G, c->cfg.head_dim,
+                                                     (const float *)c->ws_o.p,
+                                                     (const float *)c->ws_lse.p, out, lse);
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
+}  // namespace spork

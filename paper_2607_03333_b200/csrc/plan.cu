@@ -1,0 +1,303 @@
+// libspork: attention planner.
+//
+// Per fork group the DEVICE block tables decide how many leading pages all
+// members share (equal page id <=> same physical page); the host turns that and
+// its mirrored lengths into a split-KV work list:
+//   prefix segment  (one per group):  all members' rows x the shared pages, read once
+//   suffix segment  (one per member): that member's rows x its private tokens
+// Each segment is cut into equal chunks of whole 64-token tiles; one work item
+// per (chunk, kv head, block of <= 64 rows).  Items are sorted longest first.
+#include <limits.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "spork_internal.h"
+
+using namespace spork;
+
+namespace {
+
+struct GroupDesc {
+    int32_t begin, end, limit_pages, pad;
+};
+
+// one block per group: index of the first page at which the members' tables differ
+__global__ void __launch_bounds__(256) lcp_kernel(const GroupDesc *__restrict__ groups,
+                                                  const int32_t *__restrict__ seq_ids,
+                                                  const int32_t *__restrict__ table, int table_stride,
+                                                  int32_t *__restrict__ shared_out) {
+    __shared__ int s_min;
+    GroupDesc g = groups[blockIdx.x];
+    if (threadIdx.x == 0) s_min = g.limit_pages;
+    __syncthreads();
+    const int32_t *row0 = table + (size_t)seq_ids[g.begin] * table_stride;
+    for (int j = threadIdx.x; j < g.limit_pages; j += blockDim.x) {
+        int v = row0[j];
+        bool same = v >= 0;
+        for (int m = g.begin + 1; m < g.end; ++m)
+            same = same && table[(size_t)seq_ids[m] * table_stride + j] == v;
+        if (!same) atomicMin(&s_min, j);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) shared_out[blockIdx.x] = s_min;
+}
+
+constexpr int TILE_TOKENS = 64;
+constexpr int MIN_CHUNK_TILES = 4;
+constexpr int ROW_BLOCK = 64;
+
+struct Segment {
+    int table_seq, tok0, tok1;  // token range
+    int qrow0, nq;              // q rows [qrow0, qrow0 + nq)
+    int lim0;
+    int part_base, nsplit, chunk_tiles;
+    bool prefix;
+};
+
+}  // namespace
+
+namespace spork {
+
+int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
+               const int32_t *q_indptr, cudaStream_t st) {
+    Plan &P = c->plan;
+    if (n_groups < 0 || !group_indptr || group_indptr[0] != 0) return SPORK_ERR_INVALID;
+    for (int g = 0; g < n_groups; ++g)
+        if (group_indptr[g + 1] <= group_indptr[g]) return SPORK_ERR_INVALID;  // empty group
+    const int n_seq = group_indptr[n_groups];
+    if (n_seq > 0 && !seq_ids) return SPORK_ERR_INVALID;
+    const bool verify = q_indptr != nullptr;
+    for (int i = 0; i < n_seq; ++i) {
+        int s = seq_ids[i];
+        if (s < 0 || s >= c->cfg.max_seqs || !c->h_live[s]) return SPORK_ERR_INVALID_SEQ;
+    }
+    if (verify) {
+        if (q_indptr[0] != 0) return SPORK_ERR_INVALID;
+        for (int i = 0; i < n_seq; ++i) {
+            int k = q_indptr[i + 1] - q_indptr[i];
+            if (k < 1 || k > c->h_len[seq_ids[i]]) return SPORK_ERR_INVALID;
+        }
+    }
+    const int n_qrows = verify ? q_indptr[n_seq] : n_seq;
+
+    auto same = [](const std::vector<int32_t> &v, const int32_t *p, size_t n) {
+        return v.size() == n && (n == 0 || memcmp(v.data(), p, n * 4) == 0);
+    };
+    // ---- level-2 cache: nothing changed since the last call -----------------
+    if (P.valid && P.verify == verify && P.len_epoch == c->len_epoch &&
+        P.structure_epoch == c->structure_epoch && same(P.group_indptr, group_indptr, n_groups + 1) &&
+        same(P.seq_ids, seq_ids, n_seq) && (!verify || same(P.q_indptr, q_indptr, n_seq + 1))) {
+        P.info.plan_cached = 1;
+        return SPORK_OK;
+    }
+    P.valid = false;
+
+    // ---- level-1 cache: shared page counts change only with fork / release / truncate ----
+    if (!(P.shared_valid && P.shared_epoch == c->structure_epoch &&
+          same(P.shared_key_indptr, group_indptr, n_groups + 1) &&
+          same(P.shared_key_ids, seq_ids, n_seq))) {
+        P.shared_pages.assign(n_groups, 0);
+        bool any = false;
+        for (int g = 0; g < n_groups; ++g) any = any || group_indptr[g + 1] - group_indptr[g] > 1;
+        if (any) {
+            size_t bytes = sizeof(GroupDesc) * (size_t)n_groups + 4 * (size_t)n_seq + 4 * (size_t)n_groups;
+            StageSlot *slot;
+            int rc = stage_acquire(c, bytes, &slot);
+            if (rc != SPORK_OK) return rc;
+            GroupDesc *gd = (GroupDesc *)slot->h;
+            int32_t *ids = (int32_t *)(gd + n_groups);
+            for (int g = 0; g < n_groups; ++g) {
+                int lim = INT_MAX;
+                for (int i = group_indptr[g]; i < group_indptr[g + 1]; ++i)
+                    lim = std::min(lim, c->h_len[seq_ids[i]] / PS);
+                if (group_indptr[g + 1] - group_indptr[g] < 2) lim = 0;
+                gd[g] = {group_indptr[g], group_indptr[g + 1], lim, 0};
+            }
+            memcpy(ids, seq_ids, 4 * (size_t)n_seq);
+            rc = stage_commit(c, slot, bytes - 4 * (size_t)n_groups, st);
+            if (rc != SPORK_OK) return rc;
+            int32_t *d_out = (int32_t *)((char *)slot->d + bytes - 4 * (size_t)n_groups);
+            lcp_kernel<<<n_groups, 256, 0, st>>>((const GroupDesc *)slot->d,
+                                                 (const int32_t *)((GroupDesc *)slot->d + n_groups),
+                                                 c->d_table, c->table_stride, d_out);
+            c->last_launches++;
+            // documented sync: read back the per-group shared page counts
+            SPORK_CUDA(cudaMemcpyAsync(P.shared_pages.data(), d_out, 4 * (size_t)n_groups,
+                                       cudaMemcpyDeviceToHost, st));
+            SPORK_CUDA(cudaStreamSynchronize(st));
+        }
+        P.shared_valid = true;
+        P.shared_epoch = c->structure_epoch;
+        P.shared_key_indptr.assign(group_indptr, group_indptr + n_groups + 1);
+        P.shared_key_ids.assign(seq_ids, seq_ids + n_seq);
+    }
+
+    // ---- segments ------------------------------------------------------------
+    const int Hq = c->cfg.num_q_heads, Hkv = c->cfg.num_kv_heads, G = c->G;
+    std::vector<Segment> segs;
+    segs.reserve(n_groups + n_seq);
+    std::vector<QRowDesc> qd(n_qrows);
+    int64_t unique_tokens = 0, naive_tokens = 0;
+    for (int g = 0; g < n_groups; ++g) {
+        const int b = group_indptr[g], e = group_indptr[g + 1];
+        int S = P.shared_pages[g] * PS;
+        for (int i = b; i < e; ++i) {
+            int L = c->h_len[seq_ids[i]];
+            int k = verify ? q_indptr[i + 1] - q_indptr[i] : (L > 0 ? 1 : 0);
+            S = std::min(S, ((L - k) / PS) * PS);
+            naive_tokens += L;
+        }
+        if (e - b < 2 || S < 0) S = 0;
+        const int gq0 = verify ? q_indptr[b] : b;
+        const int gnq = (verify ? q_indptr[e] : e) - gq0;
+        int pre_seg = -1;
+        if (S > 0) {
+            pre_seg = (int)segs.size();
+            segs.push_back({seq_ids[b], 0, S, gq0, gnq, INT_MAX / 2, 0, 0, 0, true});
+        }
+        unique_tokens += S;
+        for (int i = b; i < e; ++i) {
+            int L = c->h_len[seq_ids[i]];
+            int q0 = verify ? q_indptr[i] : i;
+            int k = verify ? q_indptr[i + 1] - q_indptr[i] : 1;
+            int suf_seg = -1;
+            if (L > S) {
+                suf_seg = (int)segs.size();
+                segs.push_back({seq_ids[i], S, L, q0, k, L - k, 0, 0, 0, false});
+            }
+            unique_tokens += L - S;
+            for (int j = 0; j < k; ++j) {
+                QRowDesc &d = qd[q0 + j];
+                d = QRowDesc{};
+                d.pre_base = pre_seg;  // segment index for now; resolved below
+                d.pre_nq = gnq;
+                d.pre_qi = q0 + j - gq0;
+                d.suf_base = suf_seg;
+                d.suf_nq = k;
+                d.suf_qi = j;
+            }
+        }
+    }
+
+    // ---- chunking --------------------------------------------------------------
+    const bool mma = c->cfg.dtype == SPORK_BF16 && c->cfg.head_dim == 128;
+    const int grid_cap = mma ? attn_mma_grid(c) : c->num_sms * 4;
+    int64_t total_cost = 0;
+    for (const Segment &s : segs) {
+        int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
+        total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, ROW_BLOCK);
+    }
+    const int64_t target_items = (int64_t)grid_cap * 4;
+    int chunk_tiles = (int)std::max<int64_t>(MIN_CHUNK_TILES, (total_cost + target_items - 1) / target_items);
+    int64_t part_rows = 0;
+    size_t n_items = 0;
+    for (Segment &s : segs) {
+        int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
+        s.nsplit = ceil_div(tiles, chunk_tiles);
+        s.chunk_tiles = ceil_div(tiles, s.nsplit);
+        s.nsplit = ceil_div(tiles, s.chunk_tiles);
+        if (part_rows + (int64_t)s.nsplit * s.nq * Hq > INT_MAX) return SPORK_ERR_INVALID;
+        s.part_base = (int)part_rows;
+        part_rows += (int64_t)s.nsplit * s.nq * Hq;
+        n_items += (size_t)s.nsplit * Hkv * ceil_div(s.nq * G, ROW_BLOCK);
+    }
+    for (QRowDesc &d : qd) {
+        if (d.pre_base >= 0) {
+            const Segment &s = segs[d.pre_base];
+            d.pre_base = s.part_base;
+            d.pre_nsplit = s.nsplit;
+            d.pre_stride = s.nq * Hq;
+        } else {
+            d.pre_base = 0;
+            d.pre_nsplit = 0;
+        }
+        if (d.suf_base >= 0) {
+            const Segment &s = segs[d.suf_base];
+            d.suf_base = s.part_base;
+            d.suf_nsplit = s.nsplit;
+            d.suf_stride = s.nq * Hq;
+        } else {
+            d.suf_base = 0;
+            d.suf_nsplit = 0;
+        }
+    }
+
+    // ---- items, longest first ----------------------------------------------------
+    std::vector<WorkItem> items;
+    items.reserve(n_items);
+    int n_prefix_items = 0;
+    for (const Segment &s : segs) {
+        const int rows = s.nq * G;
+        for (int sp = 0; sp < s.nsplit; ++sp) {
+            int t0 = s.tok0 + sp * s.chunk_tiles * TILE_TOKENS;
+            int t1 = std::min(s.tok1, t0 + s.chunk_tiles * TILE_TOKENS);
+            for (int h = 0; h < Hkv; ++h)
+                for (int rb = 0; rb < rows; rb += ROW_BLOCK) {
+                    WorkItem it{};
+                    it.table_seq = s.table_seq;
+                    it.tok0 = t0;
+                    it.tok1 = t1;
+                    it.kvh = h;
+                    it.qrow0 = s.qrow0;
+                    it.rb0 = rb;
+                    it.nrows = std::min(ROW_BLOCK, rows - rb);
+                    it.lim0 = s.lim0;
+                    it.part_base = s.part_base + sp * s.nq * Hq + h * rows + rb;
+                    items.push_back(it);
+                    n_prefix_items += s.prefix;
+                }
+        }
+    }
+    std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
+        return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
+    });
+
+    // ---- upload (the previous plan's buffers may still be in use by queued kernels) -----------
+    if (c->plan_ev_pending) {
+        SPORK_CUDA(cudaEventSynchronize(c->plan_ev));
+        c->plan_ev_pending = false;
+    }
+    size_t ib = items.size() * sizeof(WorkItem), qb = qd.size() * sizeof(QRowDesc);
+    int rc = devbuf_reserve(&P.items, ib + 64, st);
+    if (rc == SPORK_OK) rc = devbuf_reserve(&P.qdesc, qb + 64, st);
+    if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_o, (size_t)part_rows * c->cfg.head_dim * 4 + 64, st);
+    if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_lse, (size_t)part_rows * 4 + 64, st);
+    if (rc != SPORK_OK) return rc;
+    if (ib + qb) {
+        StageSlot *slot;
+        rc = stage_acquire(c, ib + qb, &slot);
+        if (rc != SPORK_OK) return rc;
+        if (ib) memcpy(slot->h, items.data(), ib);
+        if (qb) memcpy((char *)slot->h + ib, qd.data(), qb);
+        rc = stage_commit(c, slot, ib + qb, st);
+        if (rc != SPORK_OK) return rc;
+        if (ib) SPORK_CUDA(cudaMemcpyAsync(P.items.p, slot->d, ib, cudaMemcpyDeviceToDevice, st));
+        if (qb)
+            SPORK_CUDA(cudaMemcpyAsync(P.qdesc.p, (char *)slot->d + ib, qb, cudaMemcpyDeviceToDevice, st));
+        rc = stage_done(c, slot, st);
+        if (rc != SPORK_OK) return rc;
+    }
+
+    P.n_items = (int)items.size();
+    P.n_qrows = n_qrows;
+    P.verify = verify;
+    P.len_epoch = c->len_epoch;
+    P.structure_epoch = c->structure_epoch;
+    P.group_indptr.assign(group_indptr, group_indptr + n_groups + 1);
+    P.seq_ids.assign(seq_ids, seq_ids + n_seq);
+    if (verify) P.q_indptr.assign(q_indptr, q_indptr + n_seq + 1); else P.q_indptr.clear();
+    P.info = spork_plan_info{};
+    P.info.n_items = P.n_items;
+    P.info.n_prefix_items = n_prefix_items;
+    P.info.chunk_tokens = chunk_tiles * TILE_TOKENS;
+    P.info.kernel = mma ? 1 : 0;
+    P.info.plan_cached = 0;
+    P.info.unique_tokens = unique_tokens;
+    P.info.naive_tokens = naive_tokens;
+    P.info.partial_rows = part_rows;
+    P.valid = true;
+    return SPORK_OK;
+}
+
+}  // namespace spork

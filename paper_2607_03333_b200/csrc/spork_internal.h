@@ -1,0 +1,161 @@
+// Internal declarations of libspork (CUDA path).  Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "spork.h"
+
+namespace spork {
+
+constexpr int PS = SPORK_PAGE_SIZE;  // tokens per page
+
+// ---------------------------------------------------------------------------
+// Work list (built on the host by plan.cu, consumed by the attention kernels)
+// ---------------------------------------------------------------------------
+// One item = one (segment, split, kv head, row block): `nrows` query rows
+// against tokens [tok0, tok1) of the sequence in slot `table_seq`.
+// Logical row r (rb0 <= r < rb0 + nrows) is q row (qrow0 + r / G), q head
+// (kvh * G + r % G).  Token t is visible to row r iff t <= lim0 + r / G
+// (lim0 = INT_MAX/2 for shared-prefix items: no mask).
+struct WorkItem {
+    int32_t table_seq;
+    int32_t tok0;       // multiple of 16
+    int32_t tok1;       // exclusive
+    int32_t kvh;
+    int32_t qrow0;
+    int32_t rb0;
+    int32_t nrows;      // <= 64
+    int32_t lim0;
+    int32_t part_base;  // partial row index of logical row rb0
+    int32_t pad[3];
+};
+static_assert(sizeof(WorkItem) == 48, "WorkItem layout");
+
+// Per q row: where its partials live.  Partial row index of (split s, head h):
+//   base + s * stride + (h / G) * nq * G + qi * G + h % G
+struct QRowDesc {
+    int32_t pre_base, pre_nsplit, pre_stride, pre_nq, pre_qi;
+    int32_t suf_base, suf_nsplit, suf_stride, suf_nq, suf_qi;
+    int32_t pad[2];
+};
+static_assert(sizeof(QRowDesc) == 48, "QRowDesc layout");
+
+// ---------------------------------------------------------------------------
+// staging ring: pinned host + device scratch for per-call descriptors
+// ---------------------------------------------------------------------------
+struct StageSlot {
+    void *h = nullptr;
+    void *d = nullptr;
+    size_t cap = 0;
+    cudaEvent_t ev = nullptr;
+    bool pending = false;
+};
+
+struct DevBuf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+struct Plan {
+    bool valid = false;
+    // cache keys
+    uint64_t structure_epoch = 0, len_epoch = 0;
+    bool verify = false;
+    std::vector<int32_t> group_indptr, seq_ids, q_indptr;
+    std::vector<int32_t> shared_pages;  // per group (level-1 cache)
+    bool shared_valid = false;
+    uint64_t shared_epoch = 0;
+    std::vector<int32_t> shared_key_indptr, shared_key_ids;
+    // device copies
+    DevBuf items, qdesc;
+    int n_items = 0, n_qrows = 0;
+    spork_plan_info info{};
+};
+
+}  // namespace spork
+
+struct spork_ctx {
+    spork_config cfg;
+    int G;               // Hq / Hkv
+    int elt;             // bytes per element
+    int swizzled;        // bf16 && D % 64 == 0: 128B-swizzled page-head blocks
+    size_t head_block;   // bytes of one (page, kv head) block in one pool
+    size_t page_bytes;   // bytes of one page in one pool
+    int table_stride;    // int32 per block-table row (max_pages_per_seq rounded up to 4)
+    int num_sms;
+    void *k_pool, *v_pool;
+
+    // device state
+    int32_t *d_refcount;  // [num_pages]
+    int32_t *d_table;     // [max_seqs][table_stride]
+    int32_t *d_len;       // [max_seqs]
+    int32_t *d_counters;  // [0] free pages, [1] sticky error, [2..] scratch
+    int32_t *d_free_list; // [free_list_cap] lowest free ids, ascending
+    int32_t *d_scan;      // block counts for the free-page scan
+    size_t free_list_cap;
+
+    // host mirrors (lengths and slot occupancy only; never refcounts or tables)
+    std::vector<int32_t> h_len;
+    std::vector<uint8_t> h_live;
+    std::vector<int32_t> h_shared_upto;  // pages below this index MAY be shared
+    std::vector<int32_t> h_scratch;      // per-slot scratch (fork counts, evolving lens)
+    int64_t free_lb;                     // lower bound on free pages
+    int n_live;
+
+    uint64_t structure_epoch, len_epoch;
+
+    spork::StageSlot stage[8];
+    int stage_next;
+
+    spork::Plan plan;
+    spork::DevBuf ws_o, ws_lse;   // split-KV partials
+    spork::DevBuf io_q, io_out, io_lse;  // device buffers of the *_host calls
+    void *h_io = nullptr;         // pinned bounce (unused if caller memory is pinned)
+    int last_launches;
+    cudaEvent_t plan_ev;
+    bool plan_ev_pending;
+};
+
+namespace spork {
+
+#define SPORK_CUDA(call)                                   \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return SPORK_ERR_CUDA;     \
+    } while (0)
+
+__host__ __device__ inline int ceil_div(int a, int b) { return (a + b - 1) / b; }
+__host__ __device__ inline int pages_of(int len) { return (len + PS - 1) / PS; }
+
+// staging.cu / api.cu
+int stage_acquire(spork_ctx *c, size_t bytes, StageSlot **out);           // waits for the slot
+int stage_commit(spork_ctx *c, StageSlot *s, size_t bytes, cudaStream_t st);  // H2D copy
+int stage_done(spork_ctx *c, StageSlot *s, cudaStream_t st);              // record reuse event
+int devbuf_reserve(DevBuf *b, size_t bytes, cudaStream_t st);
+
+// alloc.cu
+int launch_free_scan(spork_ctx *c, int need, cudaStream_t st);  // fills d_free_list[0..need)
+int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st);  // OOM check (may sync)
+
+// plan.cu
+int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
+               const int32_t *q_indptr, cudaStream_t st);
+
+// attention launchers
+int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st);
+int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st);
+int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st);
+int attn_mma_grid(spork_ctx *c);
+
+// element offset (in elements) of (slot r, dim d) inside one (page, kv head) block
+__host__ __device__ inline int head_block_off(int swizzled, int D, int r, int d) {
+    if (!swizzled) return r * D + d;
+    // [D/64 halves][16 rows][64 elems]; 16-byte chunk index XOR (row & 7)
+    int half = d >> 6, dd = d & 63;
+    return half * (PS * 64) + r * 64 + ((((dd >> 3) ^ (r & 7)) << 3) | (dd & 7));
+}
+
+}  // namespace spork
