@@ -1,0 +1,424 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run (the driver's contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|churn] [--k 4|8|16]
+                    [--impl reference]
+
+A step = one pass of the hot path over one batch of synthetic input:
+  configs 2/3/5  one spork_decode_attn call (plan lookup, cascade decode kernel, merge kernel)
+  config 4       one spork_verify_attn call with k drafts per sequence
+  churn          one spork_fork of 10,000 children + one spork_release of them (config 5)
+Default workload: BASELINE.json configs[1] (Qwen3-4B shape, 16 fork groups of 2, prefix 4096).
+Inputs are seeded synthetic (synth/), resident in HBM before the timed region; L2 is flushed
+between timed iterations.  `value` = unique KV bytes / step time (GB/s); config 4 also reports
+TFLOP/s.  N > 1 (torchrun) runs N independent replicas: the path does not shard ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402
+
+METRIC = "forked_decode_attn_unique_kv_bandwidth"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+# ---------------------------------------------------------------------------
+# clocks sampler (nvidia-smi during the timed region)
+# ---------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------
+# workloads
+# ---------------------------------------------------------------------------
+def pick_config(args):
+    if args.config == "churn":
+        return synth.CFG5, "cfg5_fork_churn"
+    n = int(args.config)
+    cfg = synth.CONFIGS[n]
+    if n == 4:
+        cfg = cfg.scaled(k_draft=args.k)
+        return cfg, f"cfg4_qwen3_32b_verify_k{args.k}"
+    return cfg, cfg.name
+
+
+def pool_dims(wl, num_pages=None):
+    c = wl.cfg
+    per_seq = int((wl.total_len.max() + 15) // 16) + 4
+    need = int(c.n_groups * ((c.prefix_len + 15) // 16) + sum((int(x) + 15) // 16 + 1 for x in wl.private_len))
+    return (num_pages or need + 1024), per_seq
+
+
+def build_spork(cfg, wl, num_pages=None, max_seqs=None, device="cuda:0"):
+    import paper_2607_03333_b200 as sp
+    npg, mp = pool_dims(wl, num_pages)
+    spk = sp.Spork(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, npg, max_seqs or cfg.n_seqs + 8, mp, cfg.scale,
+                   device=device)
+    ids = synth.build_state(spk, wl)
+    spk.synchronize()
+    return spk, ids
+
+
+# ---------------------------------------------------------------------------
+# the oracle leg (cpu_baseline and --impl reference): a bounded sample of the same workload
+# ---------------------------------------------------------------------------
+def oracle_sample(cfg, wl, max_groups=2):
+    """Builds `max_groups` fork groups of the workload in the CPU oracle and returns a closure that
+    runs one oracle step on them, plus the factor that scales its time to the whole batch."""
+    import oracle
+    g = min(cfg.n_groups, max_groups)
+    sub = cfg.scaled(n_groups=g)
+    # same sub-streams as the full workload: groups / sequences [0, g) are identical
+    swl = synth.Workload(sub, wl.k[:sub.n_seqs] if cfg.k_draft else None)
+    swl.suffix_len = wl.suffix_len[:sub.n_seqs].copy()
+    swl.private_len = wl.private_len[:sub.n_seqs].copy()
+    swl.total_len = wl.total_len[:sub.n_seqs].copy()
+    npg, mp = pool_dims(swl)
+    orc = oracle.Oracle(sub.dtype, sub.Hq, sub.Hkv, sub.D, npg, sub.n_seqs + 2, mp, sub.scale)
+    ids = synth.build_state(orc, swl)
+    q = swl.q_all()
+    qi = swl.q_indptr()
+    frac = float(swl.flops() / wl.flops())
+
+    def step():
+        if cfg.k_draft:
+            return orc.verify(ids, qi, q)
+        return orc.decode(ids, q)
+
+    return step, frac, oracle.num_threads(), f"{g} of {cfg.n_groups} fork groups ({sub.n_seqs} sequences), all heads"
+
+
+def run_reference(args, cfg, name, wl):
+    step, frac, cores, sample = oracle_sample(cfg, wl, args.ref_groups)
+    for _ in range(max(0, min(args.warmup, 1))):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    full = dt / frac                       # time one whole step would take, scaled by flops
+    ub = wl.unique_kv_bytes()
+    val = ub / full / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+        "config": {"workload": name, "sample": sample, "sample_seconds_per_step": dt},
+        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------
+def run_ours(args, cfg, name, wl):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    device = f"cuda:{local}"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    peaks = load_peaks()
+
+    churn = args.config == "churn"
+    num_pages = (1 << 20) if (churn or (args.config == "5" and args.full_pool)) else None
+    max_seqs = cfg.n_seqs + 10008 if churn else None
+    t_build = time.perf_counter()
+    spk, ids = build_spork(cfg, wl, num_pages, max_seqs, device)
+    t_build = time.perf_counter() - t_build
+    st = spk.stream
+    gi = wl.group_indptr()
+    qi = wl.q_indptr()
+    verify = cfg.k_draft > 0
+    q_np = wl.q_all()
+    q_dev = spk._dev(q_np)
+    rows = q_np.shape[0]
+    out = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32, device=device)
+    lse = torch.empty((rows, cfg.Hq), dtype=torch.float32, device=device)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
+    parents = synth.churn_parents(5, 10000, ids) if churn else None
+
+    churn_launches = [0]
+
+    def step():
+        if churn:
+            ch = spk.fork(parents)
+            n1 = spk.last_launches()
+            spk.release(ch)
+            churn_launches[0] = n1 + spk.last_launches()
+        elif verify:
+            spk.verify_attn(gi, ids, qi, q_dev, out, lse)
+        else:
+            spk.decode_attn(gi, ids, q_dev, out, lse)
+
+    def flush_l2():
+        with torch.cuda.stream(st):
+            flush.zero_()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(n, do_flush=True):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
+        for a, b in evs:
+            if do_flush:
+                flush_l2()
+            a.record(st)
+            step()
+            b.record(st)
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    for _ in range(max(args.warmup, 3)):
+        flush_l2()
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms = timed(args.steps)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = float(sum(ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+
+    info = spk.last_plan() if not churn else {}
+    ub = wl.unique_kv_bytes() if not churn else 0
+    flops = wl.flops()
+    launches_per_step = info.get("launches", 0) if not churn else churn_launches[0]
+
+    # ---- roofline of the dominant kernel (separate timed pass with kernel events on) ----
+    roof = None
+    extra = {}
+    if not churn:
+        spk.set_timing(True)
+        k_ms, m_ms = [], []
+        for _ in range(args.steps):
+            flush_l2()
+            step()
+            a, m = spk.last_kernel_ms()
+            k_ms.append(a)
+            m_ms.append(m)
+        spk.set_timing(False)
+        k_avg = float(np.mean(k_ms))
+        peak_bw = float(peaks["hbm_gbs"])
+        ach_bw = info["unique_tokens"] * cfg.token_bytes / (k_avg * 1e-3) / 1e9
+        peak_tf = float(peaks["bf16_tflops"])
+        ach_tf = flops / (k_avg * 1e-3) / 1e12
+        tensor_bound = verify and (flops / (peak_tf * 1e12)) > (ub / (peak_bw * 1e9))
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                traffic = json.load(f).get(name)
+        if tensor_bound:
+            roof = {"bound": "tensor", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                    "frac": ach_tf / peak_tf, "traffic": traffic}
+        else:
+            roof = {"bound": "hbm", "achieved": ach_bw, "peak": peak_bw, "unit": "GB/s",
+                    "frac": ach_bw / peak_bw, "traffic": traffic}
+        roof.update({"kernel": "attn_mma_kernel" if info["kernel"] == 1 else "attn_simt_kernel",
+                     "kernel_ms": k_avg, "merge_ms": float(np.mean(m_ms)), "peak_source": peaks["_source"],
+                     "frac_of_8TBps": ach_bw / 8000.0, "achieved_tflops": ach_tf,
+                     "algorithmic_bytes": info["unique_tokens"] * cfg.token_bytes})
+        warm = timed(args.steps, do_flush=False)
+        extra["warm_l2_ms_per_step"] = float(np.mean(warm))
+        extra["plan"] = info
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region ----
+    e2e = None
+    if not churn:
+        qh = torch.from_numpy(q_np).pin_memory()
+        oh = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32).pin_memory()
+        lh = torch.empty((rows, cfg.Hq), dtype=torch.float32).pin_memory()
+
+        def e2e_step():
+            if verify:
+                spk.verify_attn_host(gi, ids, qi, qh, oh, lh)
+            else:
+                spk.decode_attn_host(gi, ids, qh, oh, lh)
+
+        for _ in range(3):
+            e2e_step()
+        tt = []
+        for _ in range(args.steps):
+            flush_l2()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            e2e_step()
+            tt.append(time.perf_counter() - t0)
+        e_ms = float(np.mean(tt)) * 1e3
+        if world > 1:
+            t = torch.tensor([e_ms], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_ms = float(t.item())
+        e2e = {"value": world * ub / (e_ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": e_ms,
+               "h2d_bytes_per_step": int(qh.numel() * qh.element_size()),
+               "d2h_bytes_per_step": int(oh.numel() * 4 + lh.numel() * 4)}
+        # parity spot check of what was just timed (oracle, one sampled row)
+        o = oh.numpy()
+        assert np.all(np.isfinite(o))
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if not args.no_cpu_baseline and not churn:
+        ostep, frac, cores, sample = oracle_sample(cfg, wl, args.ref_groups)
+        t0 = time.perf_counter()
+        ostep()
+        dt = time.perf_counter() - t0
+        cpu = {"value": ub / (dt / frac) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+               "sample": sample, "sample_seconds": dt, "scaled_ms_per_step": dt / frac * 1e3}
+
+    if churn:
+        value, unit, metric = 10000 / (ms_step * 1e-3), "forks/s", "fork_release_churn"
+    else:
+        value, unit, metric = world * ub / (ms_step * 1e-3) / 1e9, "GB/s", METRIC
+    line = {
+        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
+        "data": "synthetic",
+        "config": {"workload": name, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_groups": cfg.n_groups,
+                   "group_size": cfg.group_size, "prefix_len": cfg.prefix_len,
+                   "suffix": [cfg.suffix_lo, cfg.suffix_hi], "k_draft": cfg.k_draft,
+                   "unique_kv_bytes": ub, "naive_kv_bytes": wl.naive_tokens() * cfg.token_bytes,
+                   "flops": flops, "l2": "flushed between timed iterations (512 MiB write)",
+                   "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "state_build_seconds": t_build},
+        "clocks": clocks,
+        "gpu_launches": int(launches_per_step * args.steps),
+        "frac_of_8TBps": (value / world / 8000.0) if not churn else None,
+        "frac_of_measured_hbm": (value / world / float(peaks["hbm_gbs"])) if not churn else None,
+    }
+    if verify:
+        line["verify_tflops"] = flops / (ms_step * 1e-3) / 1e12
+    if roof is not None:
+        line["roofline"] = roof
+    if e2e is not None:
+        line["e2e"] = e2e
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    line.update(extra)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "churn"])
+    ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-groups", type=int, default=0,
+                    help="fork groups in the oracle's bounded sample (0: per-config default)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--full-pool", action="store_true", help="config 5 on the 2^20-page pool")
+    args = ap.parse_args()
+    cfg, name = pick_config(args)
+    wl = synth.Workload(cfg)
+    if args.ref_groups <= 0:
+        args.ref_groups = {"2": 8, "3": 4, "4": 1, "5": 2, "churn": 1}[args.config]
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args, cfg, name, wl)
+        return
+    run_ours(args, cfg, name, wl)
+
+
+if __name__ == "__main__":
+    main()

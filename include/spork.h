@@ -209,6 +209,15 @@ int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
 /* kernels launched by the last state call (append / fork / release / truncate) */
 int spork_last_launches(spork_ctx *ctx);
 
+/*
+ * Kernel timing for bench.py's roofline: when enabled, the attention calls
+ * record CUDA events on `stream` around the attention kernel and around the
+ * merge kernel.  spork_last_kernel_ms synchronises on them and returns the two
+ * durations of the last call (milliseconds).  Off by default (no events).
+ */
+int spork_set_timing(spork_ctx *ctx, int enable);
+int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
+
 const char *spork_strerror(int code);
 
 #ifdef __cplusplus

@@ -32,7 +32,7 @@ ABI_SYMBOLS = [
     "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
-    "spork_strerror",
+    "spork_set_timing", "spork_last_kernel_ms", "spork_strerror",
 ]
 
 
@@ -89,6 +89,8 @@ def load(build_if_missing: bool = True):
         "spork_status": ([P], I),
         "spork_last_plan": ([P, P], I),
         "spork_last_launches": ([P], I),
+        "spork_set_timing": ([P, I], I),
+        "spork_last_kernel_ms": ([P, P, P], I),
         "spork_strerror": ([I], C.c_char_p),
     }
     for name, (args, res) in sig.items():
@@ -304,6 +306,15 @@ class Spork:
 
     def last_launches(self) -> int:
         return int(self.lib.spork_last_launches(self._h))
+
+    def set_timing(self, enable: bool):
+        self._chk(self.lib.spork_set_timing(self._h, int(bool(enable))))
+
+    def last_kernel_ms(self):
+        """(attention kernel ms, merge kernel ms) of the last attention call (synchronises)."""
+        a, m = C.c_float(), C.c_float()
+        self._chk(self.lib.spork_last_kernel_ms(self._h, C.byref(a), C.byref(m)))
+        return float(a.value), float(m.value)
 
     def synchronize(self):
         self.stream.synchronize()

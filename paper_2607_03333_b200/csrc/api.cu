@@ -177,6 +177,8 @@ extern "C" int spork_destroy(spork_ctx *c) {
                       &c->io_lse})
         if (b->p) cudaFree(b->p);
     if (c->plan_ev) cudaEventDestroy(c->plan_ev);
+    for (auto &e : c->t_ev)
+        if (e) cudaEventDestroy(e);
     delete c;
     return SPORK_OK;
 }

@@ -12,11 +12,17 @@ static int attn_common(spork_ctx *c, int n_groups, const int32_t *group_indptr, 
     Plan &P = c->plan;
     if (P.n_qrows == 0) return SPORK_OK;
     if (!q || !out || !lse) return SPORK_ERR_INVALID;
+    if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[0], st));
     rc = P.info.kernel == 1 ? launch_attn_mma(c, q, st) : launch_attn_simt(c, q, st);
     if (rc != SPORK_OK) return rc;
+    if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[1], st));
     if (P.info.kernel == 0) P.info.grid = P.n_items;
     rc = launch_merge(c, out, lse, st);
     if (rc != SPORK_OK) return rc;
+    if (c->timing) {
+        SPORK_CUDA(cudaEventRecord(c->t_ev[2], st));
+        c->t_valid = true;
+    }
     P.info.launches = c->last_launches;
     SPORK_CUDA(cudaEventRecord(c->plan_ev, st));
     c->plan_ev_pending = true;
@@ -76,4 +82,22 @@ extern "C" int spork_verify_attn_host(spork_ctx *c, int n_groups, const int32_t 
     if (!c || !q_indptr) return SPORK_ERR_INVALID;
     return attn_host(c, n_groups, group_indptr, seq_ids, q_indptr, q_host, out_host, lse_host,
                      (cudaStream_t)stream);
+}
+
+extern "C" int spork_set_timing(spork_ctx *c, int enable) {
+    if (!c) return SPORK_ERR_INVALID;
+    if (enable)
+        for (auto &e : c->t_ev)
+            if (!e) SPORK_CUDA(cudaEventCreate(&e));
+    c->timing = enable ? 1 : 0;
+    c->t_valid = false;
+    return SPORK_OK;
+}
+
+extern "C" int spork_last_kernel_ms(spork_ctx *c, float *attn_ms, float *merge_ms) {
+    if (!c || !attn_ms || !merge_ms || !c->t_valid) return SPORK_ERR_INVALID;
+    SPORK_CUDA(cudaEventSynchronize(c->t_ev[2]));
+    SPORK_CUDA(cudaEventElapsedTime(attn_ms, c->t_ev[0], c->t_ev[1]));
+    SPORK_CUDA(cudaEventElapsedTime(merge_ms, c->t_ev[1], c->t_ev[2]));
+    return SPORK_OK;
 }

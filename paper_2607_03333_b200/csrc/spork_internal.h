@@ -117,6 +117,9 @@ struct spork_ctx {
     int last_launches;
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
+    int timing = 0;
+    cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
+    bool t_valid = false;
 };
 
 namespace spork {
