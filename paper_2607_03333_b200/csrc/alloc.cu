@@ -169,8 +169,7 @@ __global__ void __launch_bounds__(256) append_copy_kernel(
         int r = pos % PS;
         size_t off;
         if (swizzled) {
-            int half = c >> 3, cc = c & 7;
-            off = (size_t)half * (PS * 128) + (size_t)r * 128 + (size_t)((cc ^ (r & 7)) << 4);
+            off = (size_t)swz_chunk_off(chunks_per_row >> 3, r, c);
         } else {
             off = ((size_t)r * chunks_per_row + c) * 16;
         }

@@ -91,7 +91,7 @@ __device__ __forceinline__ void consumer_bar() {   // the 4 consumer warps only
 
 struct Params {
     const WorkItem *items;
-    int n_items;
+    const int32_t *cta_ptr;       // this CTA runs items [cta_ptr[b], cta_ptr[b + 1])
     const uint16_t *q;
     const uint8_t *k_pool, *v_pool;
     const int32_t *table;
@@ -122,12 +122,12 @@ __device__ __forceinline__ void process_block(RowState &st, const uint32_t (&qa)
     // ---- S = Q K^T ------------------------------------------------------------
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-        const int row = ((mi >> 1) << 3) + r8;               // token row inside the page
-        const uint32_t pbase = k_base + (pg0 + p) * HEAD_BLOCK + row * 128;
+        // token row inside the page = 8 * (mi >> 1) + r8: row group (mi >> 1), row r8 of the atom
+        const uint32_t pbase = k_base + (pg0 + p) * HEAD_BLOCK + ((mi >> 1) << 11) + r8 * 128;
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {
             const int c = 2 * ks + (mi & 1);                    // 16-byte chunk 0..15
-            const uint32_t addr = pbase + ((c >> 3) << 11) + (((c & 7) ^ (row & 7)) << 4);
+            const uint32_t addr = pbase + ((c >> 3) << 10) + (((c & 7) ^ r8) << 4);
             uint32_t b0, b1, b2, b3;
             ldsm_x4(addr, b0, b1, b2, b3);
             mma_bf16(s[2 * p], qa[ks], b0, b1);
@@ -183,12 +183,11 @@ __device__ __forceinline__ void process_block(RowState &st, const uint32_t (&qa)
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
         if (p < valid_pages) {
-            const int row = ((mi & 1) << 3) + r8;
-            const uint32_t pbase = v_base + (pg0 + p) * HEAD_BLOCK + row * 128;
+            const uint32_t pbase = v_base + (pg0 + p) * HEAD_BLOCK + ((mi & 1) << 11) + r8 * 128;
 #pragma unroll
             for (int cp = 0; cp < 8; ++cp) {
                 const int c = 2 * cp + (mi >> 1);
-                const uint32_t addr = pbase + ((c >> 3) << 11) + (((c & 7) ^ (row & 7)) << 4);
+                const uint32_t addr = pbase + ((c >> 3) << 10) + (((c & 7) ^ r8) << 4);
                 uint32_t b0, b1, b2, b3;
                 ldsm_x4_t(addr, b0, b1, b2, b3);
                 mma_bf16(st.o[2 * cp], pa[p], b0, b1);
@@ -247,14 +246,15 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
     }
     __syncthreads();
 
+    // let the merge kernel's blocks become resident now; they wait for this grid to finish
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
     uint32_t stage = 0, phase = 0;   // ring position, carried across items by both roles
-    const int grid = gridDim.x, bid = blockIdx.x;
+    const int item_begin = P.cta_ptr[blockIdx.x], item_end = P.cta_ptr[blockIdx.x + 1];
 
     if (warp == N_CONSUMER_WARPS) {
         // ============================ producer ============================
-        for (int round = 0;; ++round) {
-            const int idx = round * grid + ((round & 1) ? grid - 1 - bid : bid);
-            if (idx >= P.n_items) break;
+        for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = P.items[idx];
             const int page0 = it.tok0 / PS;
             const int n_pages = (it.tok1 + PS - 1) / PS - page0;
@@ -298,9 +298,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
 
     // ================================ consumers ================================
     const int g = lane >> 2, tq = (lane & 3) * 2;
-    for (int round = 0;; ++round) {
-        const int idx = round * grid + ((round & 1) ? grid - 1 - bid : bid);
-        if (idx >= P.n_items) break;
+    for (int idx = item_begin; idx < item_end; ++idx) {
         const WorkItem it = P.items[idx];
         const int RT = it.nrows <= 16 ? 1 : (it.nrows <= 32 ? 2 : 4);   // row tiles of 16
         const int TP = N_CONSUMER_WARPS / RT;                             // token parts of a tile
@@ -358,8 +356,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
                 const int r_first = nv & (PS - 1);
                 for (int i = lane; i < (PS - r_first) * 16; i += 32) {
                     const int r = r_first + (i >> 4), c = i & 15;
-                    *reinterpret_cast<uint4 *>(vpage + ((c >> 3) << 11) + r * 128 + (((c & 7) ^ (r & 7)) << 4)) =
-                        make_uint4(0, 0, 0, 0);
+                    *reinterpret_cast<uint4 *>(vpage + swz_chunk_off(2, r, c)) = make_uint4(0, 0, 0, 0);
                 }
                 __syncwarp();
                 wrote_smem = true;
@@ -456,7 +453,7 @@ int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st) {
     }
     Params p;
     p.items = (const WorkItem *)P.items.p;
-    p.n_items = P.n_items;
+    p.cta_ptr = (const int32_t *)P.cta_ptr.p;
     p.q = (const uint16_t *)q;
     p.k_pool = (const uint8_t *)c->k_pool;
     p.v_pool = (const uint8_t *)c->v_pool;
@@ -468,7 +465,7 @@ int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st) {
     p.scale_log2 = c->cfg.scale * LOG2E;
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
-    const int grid = std::min(P.n_items, attn_mma_grid(c));
+    const int grid = P.grid;
     attn_mma_kernel<<<grid, N_THREADS, SMEM_BYTES, st>>>(p);
     c->last_launches++;
     c->plan.info.grid = grid;

@@ -21,7 +21,7 @@ __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u 
 
 // byte offset of 16-byte chunk c of row r inside a (page, kv head) block
 __device__ __forceinline__ int chunk_off(int swizzled, int chunks_per_row, int r, int c) {
-    if (swizzled) return (c >> 3) * (PS * 128) + r * 128 + (((c & 7) ^ (r & 7)) << 4);
+    if (swizzled) return swz_chunk_off(chunks_per_row >> 3, r, c);
     return (r * chunks_per_row + c) * 16;
 }
 
@@ -139,15 +139,19 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
 
 // one warp per (q row, q head): LSE-weighted combination of that row's partials
 //   M = max lse_s, w_s = exp(lse_s - M), out = sum w_s o_s / sum w_s, lse = M + ln sum w_s
-// an empty partial has lse = -inf and weight 0; no partial at all: out = 0, lse = -inf
-__global__ void __launch_bounds__(256) merge_kernel(const QRowDesc *__restrict__ qd, int n_qrows, int Hq,
-                                                    int G, int D, const float *__restrict__ ws_o,
-                                                    const float *__restrict__ ws_lse,
+// an empty partial has lse = -inf and weight 0; no partial at all: out = 0, lse = -inf.
+// Launched with programmatic stream serialisation: blocks may become resident while the
+// attention kernel still runs and wait in griddepcontrol.wait until its partials are visible.
+// Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
+// every load of a batch in flight before the first use (the kernel is pure L2 latency).
+template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
+__global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__ qd, int n_qrows, int Hq,
+                                                    int G, int D, const float *ws_o, const float *ws_lse,
                                                     float *__restrict__ out, float *__restrict__ lse) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= n_qrows * Hq) return;
     const int qrow = w / Hq, h = w % Hq, kvh = h / G, j = h % G;
-    const QRowDesc d = qd[qrow];
+    const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
     const int pre0 = d.pre_base + kvh * d.pre_nq * G + d.pre_qi * G + j;
     const int suf0 = d.suf_base + kvh * d.suf_nq * G + d.suf_qi * G + j;
     const int n = d.pre_nsplit + d.suf_nsplit;
@@ -155,35 +159,54 @@ __global__ void __launch_bounds__(256) merge_kernel(const QRowDesc *__restrict__
         return s < d.pre_nsplit ? (size_t)pre0 + (size_t)s * d.pre_stride
                                 : (size_t)suf0 + (size_t)(s - d.pre_nsplit) * d.suf_stride;
     };
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     float M = -INFINITY;
     for (int s = lane; s < n; s += 32) M = fmaxf(M, ws_lse[part(s)]);
     M = warp_max(M);
-    float *o = out + (size_t)w * D;
+    const int nv = D >> 2;                        // float4 per row (<= 64)
+    float4 *o = reinterpret_cast<float4 *>(out + (size_t)w * D);
     if (M == -INFINITY) {
-        for (int dd = lane; dd < D; dd += 32) o[dd] = 0.f;
+        for (int c = lane; c < nv; c += 32) o[c] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (lane == 0) lse[w] = -INFINITY;
         return;
     }
-    float acc[8], W = 0.f;   // D <= 256
+    float4 acc[NI];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) acc[i] = 0.f;
-    for (int s = 0; s < n; ++s) {
-        const size_t p = part(s);
-        const float ws = expf(ws_lse[p] - M);
-        if (ws == 0.f) continue;
-        W += ws;
-        const float *po = ws_o + p * D;
+    for (int i = 0; i < NI; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float W = 0.f;
+    for (int s0 = 0; s0 < n; s0 += 32) {
+        const int nb = min(32, n - s0);
+        const float wl = lane < nb ? expf(ws_lse[part(s0 + lane)] - M) : 0.f;   // weight of split s0+lane
+        for (int b0 = 0; b0 < nb; b0 += 8) {
+            float4 v[NI][8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            int dd = lane + 32 * i;
-            if (dd < D) acc[i] = fmaf(ws, po[dd], acc[i]);
+            for (int u = 0; u < 8; ++u) {
+                const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(min(s0 + b0 + u, n - 1)) * D);
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int c = lane + 32 * i;
+                    v[i][u] = c < nv ? po[c] : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float ws = __shfl_sync(0xffffffffu, wl, (b0 + u) & 31);   // 0 beyond nb
+                W += ws;
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    acc[i].x = fmaf(ws, v[i][u].x, acc[i].x);
+                    acc[i].y = fmaf(ws, v[i][u].y, acc[i].y);
+                    acc[i].z = fmaf(ws, v[i][u].z, acc[i].z);
+                    acc[i].w = fmaf(ws, v[i][u].w, acc[i].w);
+                }
+            }
         }
     }
     const float inv = 1.f / W;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        int dd = lane + 32 * i;
-        if (dd < D) o[dd] = acc[i] * inv;
+    for (int i = 0; i < NI; ++i) {
+        const int c = lane + 32 * i;
+        if (c < nv) o[c] = make_float4(acc[i].x * inv, acc[i].y * inv, acc[i].z * inv, acc[i].w * inv);
     }
     if (lane == 0) lse[w] = M + logf(W);
 }
@@ -224,10 +247,19 @@ int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_qrows == 0) return SPORK_OK;
     const int warps = P.n_qrows * c->cfg.num_q_heads;
-    merge_kernel<<<ceil_div(warps, 8), 256, 0, st>>>((const QRowDesc *)P.qdesc.p, P.n_qrows,
-                                                     c->cfg.num_q_heads, c->G, c->cfg.head_dim,
-                                                     (const float *)c->ws_o.p,
-                                                     (const float *)c->ws_lse.p, out, lse);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(ceil_div(warps, 4));
+    cfg.blockDim = dim3(128);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>,
+                                  (const QRowDesc *)P.qdesc.p, P.n_qrows,
+                                  (int)c->cfg.num_q_heads, c->G, (int)c->cfg.head_dim,
+                                  (const float *)c->ws_o.p, (const float *)c->ws_lse.p, out, lse));
     c->last_launches++;
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;

@@ -11,6 +11,9 @@
 #include <string.h>
 
 #include <algorithm>
+#include <functional>
+#include <queue>
+#include <utility>
 
 #include "spork_internal.h"
 
@@ -253,33 +256,63 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
     });
 
+    // ---- static schedule: longest-processing-time-first onto `grid` persistent CTAs ----------
+    // cost of an item = its 64-token tiles (the bytes it streams) + 1 (fixed per-item work)
+    const int grid = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
+    std::vector<int32_t> cta_ptr(grid + 1, 0);
+    if (mma && grid > 0) {
+        std::vector<int32_t> owner(items.size());
+        std::priority_queue<std::pair<int64_t, int>, std::vector<std::pair<int64_t, int>>,
+                            std::greater<std::pair<int64_t, int>>> heap;
+        for (int b = 0; b < grid; ++b) heap.push({0, b});
+        for (size_t i = 0; i < items.size(); ++i) {
+            auto top = heap.top();
+            heap.pop();
+            owner[i] = top.second;
+            cta_ptr[top.second + 1]++;
+            top.first += ceil_div(items[i].tok1 - items[i].tok0, TILE_TOKENS) + 1;
+            heap.push(top);
+        }
+        for (int b = 0; b < grid; ++b) cta_ptr[b + 1] += cta_ptr[b];
+        std::vector<int32_t> fill(cta_ptr.begin(), cta_ptr.end() - 1);
+        std::vector<WorkItem> sched(items.size());
+        for (size_t i = 0; i < items.size(); ++i) sched[fill[owner[i]]++] = items[i];
+        items.swap(sched);
+    }
+
     // ---- upload (the previous plan's buffers may still be in use by queued kernels) -----------
     if (c->plan_ev_pending) {
         SPORK_CUDA(cudaEventSynchronize(c->plan_ev));
         c->plan_ev_pending = false;
     }
     size_t ib = items.size() * sizeof(WorkItem), qb = qd.size() * sizeof(QRowDesc);
+    const size_t cb = cta_ptr.size() * 4;
     int rc = devbuf_reserve(&P.items, ib + 64, st);
     if (rc == SPORK_OK) rc = devbuf_reserve(&P.qdesc, qb + 64, st);
+    if (rc == SPORK_OK) rc = devbuf_reserve(&P.cta_ptr, cb + 64, st);
+
     if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_o, (size_t)part_rows * c->cfg.head_dim * 4 + 64, st);
     if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_lse, (size_t)part_rows * 4 + 64, st);
     if (rc != SPORK_OK) return rc;
     if (ib + qb) {
         StageSlot *slot;
-        rc = stage_acquire(c, ib + qb, &slot);
+        rc = stage_acquire(c, ib + qb + cb, &slot);
         if (rc != SPORK_OK) return rc;
         if (ib) memcpy(slot->h, items.data(), ib);
         if (qb) memcpy((char *)slot->h + ib, qd.data(), qb);
-        rc = stage_commit(c, slot, ib + qb, st);
+        memcpy((char *)slot->h + ib + qb, cta_ptr.data(), cb);
+        rc = stage_commit(c, slot, ib + qb + cb, st);
         if (rc != SPORK_OK) return rc;
         if (ib) SPORK_CUDA(cudaMemcpyAsync(P.items.p, slot->d, ib, cudaMemcpyDeviceToDevice, st));
         if (qb)
             SPORK_CUDA(cudaMemcpyAsync(P.qdesc.p, (char *)slot->d + ib, qb, cudaMemcpyDeviceToDevice, st));
+        SPORK_CUDA(cudaMemcpyAsync(P.cta_ptr.p, (char *)slot->d + ib + qb, cb, cudaMemcpyDeviceToDevice, st));
         rc = stage_done(c, slot, st);
         if (rc != SPORK_OK) return rc;
     }
 
     P.n_items = (int)items.size();
+    P.grid = grid;
     P.n_qrows = n_qrows;
     P.verify = verify;
     P.len_epoch = c->len_epoch;

@@ -71,7 +71,8 @@ struct Plan {
     std::vector<int32_t> shared_key_indptr, shared_key_ids;
     // device copies
     DevBuf items, qdesc;
-    int n_items = 0, n_qrows = 0;
+    DevBuf cta_ptr;    // int32[grid + 1]: CTA b runs items [cta_ptr[b], cta_ptr[b + 1])
+    int n_items = 0, n_qrows = 0, grid = 0;
     spork_plan_info info{};
 };
 
@@ -153,12 +154,20 @@ int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st);
 int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st);
 int attn_mma_grid(spork_ctx *c);
 
+// Swizzled (page, kv head) block, bf16 with D % 64 == 0: the block is a run of 1 KiB
+// atoms of 8 token rows x 128 bytes (64 dims), ordered [row group r/8][dim half d/64];
+// inside an atom the 16-byte chunk index is XORed with (row & 7).  This is at once the
+// conflict-free ldmatrix image and the canonical 128B-swizzle operand layout of
+// tcgen05.mma (K: K-major, V: MN-major; 8-row groups 2 * nhalf KiB apart), so one
+// bulk copy per block stages it for either tensor path.
+// byte offset of 16-byte chunk c (0 .. D/8) of token row r
+__host__ __device__ inline int swz_chunk_off(int nhalf, int r, int c) {
+    return (((r >> 3) * nhalf + (c >> 3)) << 10) + ((r & 7) << 7) + (((c & 7) ^ (r & 7)) << 4);
+}
 // element offset (in elements) of (slot r, dim d) inside one (page, kv head) block
 __host__ __device__ inline int head_block_off(int swizzled, int D, int r, int d) {
     if (!swizzled) return r * D + d;
-    // [D/64 halves][16 rows][64 elems]; 16-byte chunk index XOR (row & 7)
-    int half = d >> 6, dd = d & 63;
-    return half * (PS * 64) + r * 64 + ((((dd >> 3) ^ (r & 7)) << 3) | (dd & 7));
+    return (swz_chunk_off(D >> 6, r, d >> 3) >> 1) + (d & 7);
 }
 
 }  // namespace spork
