@@ -208,6 +208,8 @@ def run_ours(args, cfg, name, wl):
     t_build = time.perf_counter()
     spk, ids = build_spork(cfg, wl, num_pages, max_seqs, device)
     t_build = time.perf_counter() - t_build
+    if args.min_rows is not None:
+        spk.set_tensor_path_min_rows(args.min_rows)
     st = spk.stream
     gi = wl.group_indptr()
     qi = wl.q_indptr()
@@ -309,7 +311,9 @@ def run_ours(args, cfg, name, wl):
         else:
             roof = {"bound": "hbm", "achieved": ach_bw, "peak": peak_bw, "unit": "GB/s",
                     "frac": ach_bw / peak_bw, "traffic": traffic}
-        roof.update({"kernel": "attn_mma_kernel" if info["kernel"] == 1 else "attn_simt_kernel",
+        kname = {0: "attn_simt_kernel", 1: "attn_mma_kernel", 2: "attn_umma_kernel",
+                 3: "attn_umma_kernel+attn_mma_kernel"}[info["kernel"]]
+        roof.update({"kernel": kname,
                      "kernel_ms": k_avg, "merge_ms": float(np.mean(m_ms)), "peak_source": peaks["_source"],
                      "frac_of_8TBps": ach_bw / 8000.0, "achieved_tflops": ach_tf,
                      "algorithmic_bytes": info["unique_tokens"] * cfg.token_bytes})
@@ -411,6 +415,8 @@ def main():
     ap.add_argument("--ref-groups", type=int, default=0,
                     help="fork groups in the oracle's bounded sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--min-rows", type=int, default=None,
+                    help="planner knob: rows per KV head from which a segment runs on the tcgen05 kernel")
     ap.add_argument("--full-pool", action="store_true", help="config 5 on the 2^20-page pool")
     args = ap.parse_args()
     cfg, name = pick_config(args)

@@ -197,13 +197,14 @@ typedef struct spork_plan_info {
     int32_t n_prefix_items; /* of which shared-prefix items                         */
     int32_t chunk_tokens;   /* split-KV chunk length                                */
     int32_t grid;           /* CTAs launched by the attention kernel                */
-    int32_t kernel;         /* 0 = simt (fp32 / generic), 1 = mma (bf16, D = 128)    */
+    int32_t kernel;         /* 0 = simt (fp32 / generic); bf16, D = 128: 1 = mma.sync,
+                               2 = tcgen05, 3 = both (many-row items on tcgen05)     */
     int32_t plan_cached;    /* 1 if the last call reused the previous plan          */
     int64_t unique_tokens;  /* sum_groups (shared + sum_members private) tokens     */
     int64_t naive_tokens;   /* sum_members len                                      */
     int64_t partial_rows;   /* rows of split-KV workspace written                   */
     int32_t launches;       /* kernels launched by the last attention call          */
-    int32_t reserved;
+    int32_t n_umma_items;   /* of n_items, those run by the tcgen05 kernel          */
 } spork_plan_info;
 int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
 /* kernels launched by the last state call (append / fork / release / truncate) */
@@ -217,6 +218,16 @@ int spork_last_launches(spork_ctx *ctx);
  */
 int spork_set_timing(spork_ctx *ctx, int enable);
 int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
+
+/*
+ * Tuning knob of the planner (bf16, D = 128 contexts only): a segment -- a fork group's shared
+ * prefix or one sequence's private tail -- whose query rows x GQA heads per KV head number at
+ * least `min_rows` is run by the tcgen05 (TMEM) kernel in row blocks of 128, the others by the
+ * mma.sync kernel.  Default 33.  min_rows <= 1 sends everything to the tcgen05 kernel, a value
+ * above 128 * max rows nothing.  Results do not depend on it beyond rounding.  Invalidates the
+ * cached plan.  SPORK_ERR_INVALID on a null context.
+ */
+int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
 
 const char *spork_strerror(int code);
 

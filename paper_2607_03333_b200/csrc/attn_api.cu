@@ -13,10 +13,18 @@ static int attn_common(spork_ctx *c, int n_groups, const int32_t *group_indptr, 
     if (P.n_qrows == 0) return SPORK_OK;
     if (!q || !out || !lse) return SPORK_ERR_INVALID;
     if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[0], st));
-    rc = P.info.kernel == 1 ? launch_attn_mma(c, q, st) : launch_attn_simt(c, q, st);
+    if (P.info.kernel == 0) {
+        rc = launch_attn_simt(c, q, st);
+    } else {
+        // many-row items on the tcgen05 kernel first (the long shared-prefix streams), then the
+        // few-row items on the mma.sync kernel, which is allowed to start while the first drains
+        rc = launch_attn_umma(c, q, st);
+        if (rc == SPORK_OK) rc = launch_attn_mma(c, q, st);
+    }
     if (rc != SPORK_OK) return rc;
     if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[1], st));
     if (P.info.kernel == 0) P.info.grid = P.n_items;
+    if (P.info.kernel == 2) P.info.grid = P.grid_umma;
     rc = launch_merge(c, out, lse, st);
     if (rc != SPORK_OK) return rc;
     if (c->timing) {
@@ -99,5 +107,12 @@ extern "C" int spork_last_kernel_ms(spork_ctx *c, float *attn_ms, float *merge_m
     SPORK_CUDA(cudaEventSynchronize(c->t_ev[2]));
     SPORK_CUDA(cudaEventElapsedTime(attn_ms, c->t_ev[0], c->t_ev[1]));
     SPORK_CUDA(cudaEventElapsedTime(merge_ms, c->t_ev[1], c->t_ev[2]));
+    return SPORK_OK;
+}
+
+extern "C" int spork_set_tensor_path_min_rows(spork_ctx *c, int min_rows) {
+    if (!c) return SPORK_ERR_INVALID;
+    c->umma_min_rows = min_rows;
+    c->plan.valid = false;
     return SPORK_OK;
 }

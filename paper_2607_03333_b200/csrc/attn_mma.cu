@@ -434,6 +434,10 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
             }
         }
     }
+    // When launched programmatically behind the tcgen05 kernel this grid may start before that one
+    // has finished; do not complete before it has, so that merge_kernel (which waits for THIS grid)
+    // sees both kernels' partials.  A no-op for a normal launch.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace
@@ -466,7 +470,17 @@ int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st) {
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
     const int grid = P.grid;
-    attn_mma_kernel<<<grid, N_THREADS, SMEM_BYTES, st>>>(p);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(N_THREADS);
+    cfg.dynamicSmemBytes = SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = P.n_items_umma > 0 ? 1 : 0;   // overlap the tail of the tcgen05 kernel
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_mma_kernel, p));
     c->last_launches++;
     c->plan.info.grid = grid;
     SPORK_CUDA(cudaGetLastError());

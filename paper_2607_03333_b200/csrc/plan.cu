@@ -6,7 +6,11 @@
 //   prefix segment  (one per group):  all members' rows x the shared pages, read once
 //   suffix segment  (one per member): that member's rows x its private tokens
 // Each segment is cut into equal chunks of whole 64-token tiles; one work item
-// per (chunk, kv head, block of <= 64 rows).  Items are sorted longest first.
+// per (chunk, kv head, row block).  Segments with many rows (>= umma_min_rows: the GQA
+// heads of a whole fork group, or a verify call's drafts) go to the tcgen05 kernel in
+// row blocks of <= 128; the others to the mma.sync kernel in row blocks of <= 64.
+// Each kernel's items are sorted longest first and statically scheduled onto its
+// persistent CTAs.
 #include <limits.h>
 #include <string.h>
 
@@ -49,6 +53,7 @@ __global__ void __launch_bounds__(256) lcp_kernel(const GroupDesc *__restrict__ 
 constexpr int TILE_TOKENS = 64;
 constexpr int MIN_CHUNK_TILES = 4;
 constexpr int ROW_BLOCK = 64;
+constexpr int ROW_BLOCK_UMMA = 128;
 
 struct Segment {
     int table_seq, tok0, tok1;  // token range
@@ -56,7 +61,36 @@ struct Segment {
     int lim0;
     int part_base, nsplit, chunk_tiles;
     bool prefix;
+    bool umma;
+    int row_block;
 };
+
+// longest first, then longest-processing-time-first onto `grid` persistent CTAs;
+// cost of an item = its 64-token tiles (the bytes it streams) + 1 (fixed per-item work)
+void schedule(std::vector<WorkItem> &items, int grid, std::vector<int32_t> &cta_ptr) {
+    std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
+        return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
+    });
+    cta_ptr.assign(grid + 1, 0);
+    if (grid == 0) return;
+    std::vector<int32_t> owner(items.size());
+    std::priority_queue<std::pair<int64_t, int>, std::vector<std::pair<int64_t, int>>,
+                        std::greater<std::pair<int64_t, int>>> heap;
+    for (int b = 0; b < grid; ++b) heap.push({0, b});
+    for (size_t i = 0; i < items.size(); ++i) {
+        auto top = heap.top();
+        heap.pop();
+        owner[i] = top.second;
+        cta_ptr[top.second + 1]++;
+        top.first += ceil_div(items[i].tok1 - items[i].tok0, TILE_TOKENS) + 1;
+        heap.push(top);
+    }
+    for (int b = 0; b < grid; ++b) cta_ptr[b + 1] += cta_ptr[b];
+    std::vector<int32_t> fill(cta_ptr.begin(), cta_ptr.end() - 1);
+    std::vector<WorkItem> sched(items.size());
+    for (size_t i = 0; i < items.size(); ++i) sched[fill[owner[i]]++] = items[i];
+    items.swap(sched);
+}
 
 }  // namespace
 
@@ -157,7 +191,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         int pre_seg = -1;
         if (S > 0) {
             pre_seg = (int)segs.size();
-            segs.push_back({seq_ids[b], 0, S, gq0, gnq, INT_MAX / 2, 0, 0, 0, true});
+            segs.push_back({seq_ids[b], 0, S, gq0, gnq, INT_MAX / 2, 0, 0, 0, true, false, ROW_BLOCK});
         }
         unique_tokens += S;
         for (int i = b; i < e; ++i) {
@@ -167,7 +201,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             int suf_seg = -1;
             if (L > S) {
                 suf_seg = (int)segs.size();
-                segs.push_back({seq_ids[i], S, L, q0, k, L - k, 0, 0, 0, false});
+                segs.push_back({seq_ids[i], S, L, q0, k, L - k, 0, 0, 0, false, false, ROW_BLOCK});
             }
             unique_tokens += L - S;
             for (int j = 0; j < k; ++j) {
@@ -187,9 +221,11 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     const bool mma = c->cfg.dtype == SPORK_BF16 && c->cfg.head_dim == 128;
     const int grid_cap = mma ? attn_mma_grid(c) : c->num_sms * 4;
     int64_t total_cost = 0;
-    for (const Segment &s : segs) {
+    for (Segment &s : segs) {
+        s.umma = mma && s.nq * G >= c->umma_min_rows;
+        s.row_block = s.umma ? ROW_BLOCK_UMMA : ROW_BLOCK;
         int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
-        total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, ROW_BLOCK);
+        total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, s.row_block);
     }
     const int64_t target_items = (int64_t)grid_cap * 4;
     int chunk_tiles = (int)std::max<int64_t>(MIN_CHUNK_TILES, (total_cost + target_items - 1) / target_items);
@@ -203,7 +239,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         if (part_rows + (int64_t)s.nsplit * s.nq * Hq > INT_MAX) return SPORK_ERR_INVALID;
         s.part_base = (int)part_rows;
         part_rows += (int64_t)s.nsplit * s.nq * Hq;
-        n_items += (size_t)s.nsplit * Hkv * ceil_div(s.nq * G, ROW_BLOCK);
+        n_items += (size_t)s.nsplit * Hkv * ceil_div(s.nq * G, s.row_block);
     }
     for (QRowDesc &d : qd) {
         if (d.pre_base >= 0) {
@@ -226,17 +262,18 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         }
     }
 
-    // ---- items, longest first ----------------------------------------------------
-    std::vector<WorkItem> items;
+    // ---- items of the two kernels, each longest first and statically scheduled -----------------
+    std::vector<WorkItem> items, items_umma;
     items.reserve(n_items);
     int n_prefix_items = 0;
     for (const Segment &s : segs) {
         const int rows = s.nq * G;
+        std::vector<WorkItem> &dst = s.umma ? items_umma : items;
         for (int sp = 0; sp < s.nsplit; ++sp) {
             int t0 = s.tok0 + sp * s.chunk_tiles * TILE_TOKENS;
             int t1 = std::min(s.tok1, t0 + s.chunk_tiles * TILE_TOKENS);
             for (int h = 0; h < Hkv; ++h)
-                for (int rb = 0; rb < rows; rb += ROW_BLOCK) {
+                for (int rb = 0; rb < rows; rb += s.row_block) {
                     WorkItem it{};
                     it.table_seq = s.table_seq;
                     it.tok0 = t0;
@@ -244,41 +281,30 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
                     it.kvh = h;
                     it.qrow0 = s.qrow0;
                     it.rb0 = rb;
-                    it.nrows = std::min(ROW_BLOCK, rows - rb);
+                    it.nrows = std::min(s.row_block, rows - rb);
                     it.lim0 = s.lim0;
                     it.part_base = s.part_base + sp * s.nq * Hq + h * rows + rb;
-                    items.push_back(it);
+                    dst.push_back(it);
                     n_prefix_items += s.prefix;
                 }
         }
     }
-    std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
-        return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
-    });
-
-    // ---- static schedule: longest-processing-time-first onto `grid` persistent CTAs ----------
-    // cost of an item = its 64-token tiles (the bytes it streams) + 1 (fixed per-item work)
     const int grid = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
-    std::vector<int32_t> cta_ptr(grid + 1, 0);
-    if (mma && grid > 0) {
-        std::vector<int32_t> owner(items.size());
-        std::priority_queue<std::pair<int64_t, int>, std::vector<std::pair<int64_t, int>>,
-                            std::greater<std::pair<int64_t, int>>> heap;
-        for (int b = 0; b < grid; ++b) heap.push({0, b});
-        for (size_t i = 0; i < items.size(); ++i) {
-            auto top = heap.top();
-            heap.pop();
-            owner[i] = top.second;
-            cta_ptr[top.second + 1]++;
-            top.first += ceil_div(items[i].tok1 - items[i].tok0, TILE_TOKENS) + 1;
-            heap.push(top);
-        }
-        for (int b = 0; b < grid; ++b) cta_ptr[b + 1] += cta_ptr[b];
-        std::vector<int32_t> fill(cta_ptr.begin(), cta_ptr.end() - 1);
-        std::vector<WorkItem> sched(items.size());
-        for (size_t i = 0; i < items.size(); ++i) sched[fill[owner[i]]++] = items[i];
-        items.swap(sched);
+    const int grid_umma = (int)std::min<size_t>(items_umma.size(), (size_t)attn_umma_grid(c));
+    std::vector<int32_t> cta_ptr, cta_ptr_umma;
+    if (mma) {
+        schedule(items, grid, cta_ptr);
+        schedule(items_umma, grid_umma, cta_ptr_umma);
+    } else {
+        std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
+            return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
+        });
+        cta_ptr.assign(grid + 1, 0);
+        cta_ptr_umma.assign(1, 0);
     }
+    const int n_items_mma = (int)items.size();
+    items.insert(items.end(), items_umma.begin(), items_umma.end());
+    cta_ptr.insert(cta_ptr.end(), cta_ptr_umma.begin(), cta_ptr_umma.end());
 
     // ---- upload (the previous plan's buffers may still be in use by queued kernels) -----------
     if (c->plan_ev_pending) {
@@ -311,8 +337,10 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         if (rc != SPORK_OK) return rc;
     }
 
-    P.n_items = (int)items.size();
+    P.n_items = n_items_mma;
+    P.n_items_umma = (int)items.size() - n_items_mma;
     P.grid = grid;
+    P.grid_umma = grid_umma;
     P.n_qrows = n_qrows;
     P.verify = verify;
     P.len_epoch = c->len_epoch;
@@ -321,10 +349,11 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     P.seq_ids.assign(seq_ids, seq_ids + n_seq);
     if (verify) P.q_indptr.assign(q_indptr, q_indptr + n_seq + 1); else P.q_indptr.clear();
     P.info = spork_plan_info{};
-    P.info.n_items = P.n_items;
+    P.info.n_items = P.n_items + P.n_items_umma;
+    P.info.n_umma_items = P.n_items_umma;
     P.info.n_prefix_items = n_prefix_items;
     P.info.chunk_tokens = chunk_tiles * TILE_TOKENS;
-    P.info.kernel = mma ? 1 : 0;
+    P.info.kernel = !mma ? 0 : (P.n_items_umma == 0 ? 1 : (P.n_items == 0 ? 2 : 3));
     P.info.plan_cached = 0;
     P.info.unique_tokens = unique_tokens;
     P.info.naive_tokens = naive_tokens;

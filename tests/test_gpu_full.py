@@ -54,7 +54,7 @@ def test_full_decode_configs(n):
     _state_properties(spk, wl, ids)
     out, lse = spk.decode_attn(wl.group_indptr(), ids, wl.q_all())
     info = spk.last_plan()
-    assert info["kernel"] == 1 and info["unique_tokens"] == wl.unique_tokens()
+    assert info["kernel"] in (1, 2, 3) and info["unique_tokens"] == wl.unique_tokens()
     assert info["n_prefix_items"] > 0
     sampled_rows_check(out, lse, wl, _samples(wl, 6, n), cfg.name)
     assert np.all(np.isfinite(out.cpu().numpy()))

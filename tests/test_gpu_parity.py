@@ -92,16 +92,36 @@ SMALL_DECODE = [
 ]
 
 
+# planner knob: which segments run on the tcgen05 kernel (None = default threshold)
+PATHS = {"auto": None, "tcgen05": 1, "mma.sync": 1 << 20}
+
+
+def _set_path(spk, path):
+    if PATHS[path] is not None:
+        spk.set_tensor_path_min_rows(PATHS[path])
+
+
+def _check_kernel(info, path):
+    if path == "tcgen05":
+        assert info["kernel"] == 2 and info["n_umma_items"] == info["n_items"]
+    elif path == "mma.sync":
+        assert info["kernel"] == 1 and info["n_umma_items"] == 0
+    else:
+        assert info["kernel"] in (1, 2, 3)
+
+
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("cfg", SMALL_DECODE, ids=lambda c: f"{c.name}-g{c.group_size}-P{c.prefix_len}")
-def test_small_bf16_decode(cfg):
+def test_small_bf16_decode(cfg, path):
     wl, orc, spk, ids = _build_both(cfg)
+    _set_path(spk, path)
     assert_state_equal(orc, spk, ids)
     q = wl.q_all()
     out_ref, lse_ref = orc.decode(ids, q)
     out, lse = spk.decode_attn(wl.group_indptr(), ids, q)
     check_attn(out, lse, out_ref, lse_ref, "bf16", cfg.name)
     info = spk.last_plan()
-    assert info["kernel"] == 1
+    _check_kernel(info, path)
     # an unaligned fork point duplicates the tail page: those tokens are private copies
     dup = cfg.n_groups * (cfg.group_size - 1) * (cfg.prefix_len % 16)
     assert info["unique_tokens"] == wl.unique_tokens() + dup
@@ -131,16 +151,19 @@ def test_small_fp32_generic_paths():
 # ---------------------------------------------------------------------------
 # verify (config 4 shape, scaled): mixed k, causal within the drafts
 # ---------------------------------------------------------------------------
+@pytest.mark.parametrize("path", list(PATHS))
 @pytest.mark.parametrize("ks", [[4, 8, 16, 1], [16, 16, 16, 16], [1, 1, 1, 1], [3, 7, 12, 5]])
-def test_small_verify(ks):
+def test_small_verify(ks, path):
     cfg = synth.CFG4.scaled(n_groups=2, prefix_len=1024 + 32, suffix_lo=0, suffix_hi=100)
     kk = np.array(ks * cfg.n_groups)
     wl, orc, spk, ids = _build_both(cfg, kk)
+    _set_path(spk, path)
     assert_state_equal(orc, spk, ids)
     q, qi = wl.q_all(), wl.q_indptr()
     out_ref, lse_ref = orc.verify(ids, qi, q)
     out, lse = spk.verify_attn(wl.group_indptr(), ids, qi, q)
     check_attn(out, lse, out_ref, lse_ref, "bf16", f"verify k={ks}")
+    _check_kernel(spk.last_plan(), path)
     # ungrouped = same result
     out1, lse1 = spk.verify_attn(np.arange(len(ids) + 1), ids, qi, q)
     check_attn(out1, lse1, out_ref, lse_ref, "bf16", f"verify ungrouped k={ks}")
