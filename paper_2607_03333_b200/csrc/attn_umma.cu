@@ -31,7 +31,7 @@ constexpr int TILE_PAGES = 4;
 constexpr int TILE_TOKENS = TILE_PAGES * PS;          // 64
 constexpr int HEAD_BLOCK = PS * D * 2;                // 4096 B: one (page, kv head) block
 constexpr int SLOT_BYTES = TILE_PAGES * HEAD_BLOCK;   // 16 KiB: a K tile or a V tile
-constexpr int NSLOT = 4;
+constexpr int NSLOT = 5;
 constexpr int Q_BYTES = 128 * D * 2;                  // 32 KiB
 constexpr int Q_HALF = Q_BYTES / 2;                   // dims [64, 128) start here
 constexpr int N_THREADS = 192;
