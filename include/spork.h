@@ -223,8 +223,9 @@ int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
  * Tuning knob of the planner (bf16, D = 128 contexts only): a segment -- a fork group's shared
  * prefix or one sequence's private tail -- whose query rows x GQA heads per KV head number at
  * least `min_rows` is run by the tcgen05 (TMEM) kernel in row blocks of 128, the others by the
- * mma.sync kernel.  Default 33.  min_rows <= 1 sends everything to the tcgen05 kernel, a value
- * above 128 * max rows nothing.  Results do not depend on it beyond rounding.  Invalidates the
+ * mma.sync kernel.  Default 1: everything runs on the tcgen05 kernel (measured at least as fast
+ * as any split on every BASELINE.json config); a value above the largest row count sends
+ * everything to the mma.sync kernel.  Results do not depend on it beyond rounding.  Invalidates the
  * cached plan.  SPORK_ERR_INVALID on a null context.
  */
 int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);

@@ -236,7 +236,24 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
             }
             const int lim_r = it.lim0 + (it.rb0 + r) / P.G;
             const int min_lim = it.lim0 + it.rb0 / P.G;
-            float m_used = -INFINITY, l = 0.f;
+            float m_used = -INFINITY, l = 0.f, lr = 0.f;   // l: exact row sum (lse); lr: sum of the bf16 weights
+
+            if (lg * 32 >= it.nrows) {
+                // none of this warp's 32 rows exists (few-row item): only keep the barriers moving;
+                // whatever S/P/O hold in these lanes never leaves TMEM
+                for (int i = 0; i < n_tiles; ++i) {
+                    const uint32_t g = g0 + i, b = g & 1;
+                    mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
+                    if (lane == 0) mbar_arrive(bar(B_PFULL + b));
+                    __syncwarp();
+                }
+                const uint32_t gl = g0 + n_tiles - 1;
+                mbar_wait(bar(B_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                if (lane == 0) mbar_arrive(bar(B_OFREE));
+                __syncwarp();
+                g0 += n_tiles;
+                continue;
+            }
 
             for (int i = 0; i < n_tiles; ++i) {
                 const uint32_t g = g0 + i, b = g & 1;
@@ -267,6 +284,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                     const float m_new = grow ? mxs : m_used;
                     const float alpha = grow ? (m_used == -INFINITY ? 0.f : ex2(m_used - m_new)) : 1.f;
                     l *= alpha;
+                    lr *= alpha;
                     if (i > 0) {
                         // O holds tiles [0, i): wait for P V(i - 1), rescale this thread's row
                         mbar_wait(bar(B_PVDONE + ((g - 1) & 1)), ((g - 1) >> 1) & 1);
@@ -286,30 +304,38 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                 }
                 const float mu = m_used == -INFINITY ? 0.f : m_used;
                 uint32_t p[32];
-                float sum0 = 0.f, sum1 = 0.f;
+                float sum0 = 0.f, sum1 = 0.f, rs0 = 0.f, rs1 = 0.f;
 #pragma unroll
                 for (int t = 0; t < 16; ++t) {
                     const float a0 = ex2(fmaf(__uint_as_float(s0[2 * t]), P.scale_log2, -mu));
                     const float a1 = ex2(fmaf(__uint_as_float(s0[2 * t + 1]), P.scale_log2, -mu));
                     const float c0 = ex2(fmaf(__uint_as_float(s1[2 * t]), P.scale_log2, -mu));
                     const float c1 = ex2(fmaf(__uint_as_float(s1[2 * t + 1]), P.scale_log2, -mu));
-                    sum0 += a0 + a1;
-                    sum1 += c0 + c1;
                     p[t] = pack_bf16(a0, a1);
                     p[16 + t] = pack_bf16(c0, c1);
+                    // o is normalised by the sum of the ROUNDED weights the tensor core uses, so that
+                    // o = sum(p v) / sum(p) stays a true weighted mean (a one-hot row returns V exactly
+                    // even when the running max is stale and p is not a power of two); lse keeps the
+                    // exact sum
+                    sum0 += a0 + a1;
+                    sum1 += c0 + c1;
+                    rs0 += __uint_as_float(p[t] << 16) + __uint_as_float(p[t] & 0xffff0000u);
+                    rs1 += __uint_as_float(p[16 + t] << 16) + __uint_as_float(p[16 + t] & 0xffff0000u);
                 }
                 l += sum0 + sum1;
+                lr += rs0 + rs1;
                 tmem_st32(tS, p);
                 tmem_wait_st();
-                if (nv & (PS - 1)) {
+                if ((nv & (PS - 1)) && lg == 0) {
                     // the last staged page is partially filled: its tail rows hold whatever the pool
-                    // held (possibly NaN patterns).  P is 0 there; make V 0 as well.
+                    // held (possibly NaN patterns).  P is 0 there; make V 0 as well (the warp of rows
+                    // 0..31 does it: it is active in every item).
                     const uint32_t ldv = 2 * g + 1, slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
                     mbar_wait(bar(B_FULL + slot), ph);
                     const int nvp = (nv + PS - 1) / PS;
                     uint8_t *vpage = smem + Q_BYTES + slot * SLOT_BYTES + (nvp - 1) * HEAD_BLOCK;
                     const int r_first = nv & (PS - 1);
-                    for (int e = st; e < (PS - r_first) * 16; e += 128) {
+                    for (int e = lane; e < (PS - r_first) * 16; e += 32) {
                         const int rr = r_first + (e >> 4), cc = e & 15;
                         *reinterpret_cast<uint4 *>(vpage + swz_chunk_off(2, rr, cc)) = make_uint4(0, 0, 0, 0);
                     }
@@ -325,7 +351,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                 const uint32_t gl = g0 + n_tiles - 1;
                 mbar_wait(bar(B_PVDONE + (gl & 1)), (gl >> 1) & 1);
                 tc_fence_after();
-                const float inv = l > 0.f ? 1.f / l : 0.f;
+                const float inv = lr > 0.f ? 1.f / lr : 0.f;
                 float *dst = P.ws_o + (size_t)(it.part_base + r) * D;
 #pragma unroll 1
                 for (int cb = 0; cb < 4; ++cb) {

@@ -54,6 +54,8 @@ constexpr int TILE_TOKENS = 64;
 constexpr int MIN_CHUNK_TILES = 4;
 constexpr int ROW_BLOCK = 64;
 constexpr int ROW_BLOCK_UMMA = 128;
+constexpr float ITEM_FIXED_COST = 1.5f;        // per-item overhead in 64-token-tile times
+constexpr float ITEM_FIXED_COST_UMMA = 4.f;    // ... of the tcgen05 kernel (32 KiB of Q, 64 KiB of partials)
 
 struct Segment {
     int table_seq, tok0, tok1;  // token range
@@ -82,7 +84,7 @@ void schedule(std::vector<WorkItem> &items, int grid, std::vector<int32_t> &cta_
         heap.pop();
         owner[i] = top.second;
         cta_ptr[top.second + 1]++;
-        top.first += ceil_div(items[i].tok1 - items[i].tok0, TILE_TOKENS) + 1;
+        top.first += 2 * ceil_div(items[i].tok1 - items[i].tok0, TILE_TOKENS) + 3;   // 2 x (tiles + 1.5)
         heap.push(top);
     }
     for (int b = 0; b < grid; ++b) cta_ptr[b + 1] += cta_ptr[b];
@@ -227,19 +229,81 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
         total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, s.row_block);
     }
-    const int64_t target_items = (int64_t)grid_cap * 4;
-    int chunk_tiles = (int)std::max<int64_t>(MIN_CHUNK_TILES, (total_cost + target_items - 1) / target_items);
+    // ---- split-KV chunk length: the candidate that minimises the estimated step time --------
+    // Unit = the time one CTA needs to stream a 64-token tile when every CTA is busy.  An item
+    // costs its tiles plus a fixed part (Q staging, partial write-back); the partials are written
+    // once and read once by the merge kernel, which all CTAs share.  Fewer, longer items cost less
+    // overhead and less partial traffic; more, shorter items balance the persistent CTAs better.
+    const int grid_cap_umma = mma ? attn_umma_grid(c) : 0;
+    auto split = [&](int chunk_tiles, int64_t *part_rows_out, size_t *n_items_out) -> bool {
+        int64_t part_rows = 0;
+        size_t n_items = 0;
+        for (Segment &s : segs) {
+            int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
+            s.nsplit = ceil_div(tiles, chunk_tiles);
+            s.chunk_tiles = ceil_div(tiles, s.nsplit);
+            s.nsplit = ceil_div(tiles, s.chunk_tiles);
+            if (part_rows + (int64_t)s.nsplit * s.nq * Hq > INT_MAX) return false;
+            s.part_base = (int)part_rows;
+            part_rows += (int64_t)s.nsplit * s.nq * Hq;
+            n_items += (size_t)s.nsplit * Hkv * ceil_div(s.nq * G, s.row_block);
+        }
+        *part_rows_out = part_rows;
+        *n_items_out = n_items;
+        return true;
+    };
+    auto makespan = [&](bool umma, int grid) -> double {
+        std::vector<float> cost;
+        for (const Segment &s : segs) {
+            if (s.umma != umma) continue;
+            const int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
+            const int n_rb = ceil_div(s.nq * G, s.row_block);
+            for (int sp = 0; sp < s.nsplit; ++sp) {
+                const float t = (float)std::min(s.chunk_tiles, tiles - sp * s.chunk_tiles) +
+                                (umma ? ITEM_FIXED_COST_UMMA : ITEM_FIXED_COST);
+                cost.insert(cost.end(), (size_t)Hkv * n_rb, t);
+            }
+        }
+        if (cost.empty()) return 0.0;
+        std::sort(cost.begin(), cost.end(), std::greater<float>());
+        const int g = (int)std::min<size_t>(cost.size(), (size_t)grid);
+        std::priority_queue<double, std::vector<double>, std::greater<double>> heap;
+        for (int b = 0; b < g; ++b) heap.push(0.0);
+        double mk = 0.0;
+        for (float t : cost) {
+            double v = heap.top() + t;
+            heap.pop();
+            heap.push(v);
+            mk = std::max(mk, v);
+        }
+        return mk;
+    };
+    int chunk_tiles = MIN_CHUNK_TILES;
     int64_t part_rows = 0;
     size_t n_items = 0;
-    for (Segment &s : segs) {
-        int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
-        s.nsplit = ceil_div(tiles, chunk_tiles);
-        s.chunk_tiles = ceil_div(tiles, s.nsplit);
-        s.nsplit = ceil_div(tiles, s.chunk_tiles);
-        if (part_rows + (int64_t)s.nsplit * s.nq * Hq > INT_MAX) return SPORK_ERR_INVALID;
-        s.part_base = (int)part_rows;
-        part_rows += (int64_t)s.nsplit * s.nq * Hq;
-        n_items += (size_t)s.nsplit * Hkv * ceil_div(s.nq * G, s.row_block);
+    {
+        static const float mult[] = {1.f, 1.5f, 2.f, 3.f, 4.f, 6.f};
+        double best = -1.0;
+        int best_chunk = -1;
+        const int row_bytes = c->cfg.head_dim * 4 + 4;
+        const double tile_bytes = 2.0 * TILE_TOKENS * c->cfg.head_dim * c->elt;
+        for (float m : mult) {
+            const int64_t target = (int64_t)(grid_cap * m);
+            const int ct = (int)std::max<int64_t>(MIN_CHUNK_TILES, (total_cost + target - 1) / target);
+            if (ct == best_chunk) continue;
+            int64_t pr;
+            size_t ni;
+            if (!split(ct, &pr, &ni)) continue;
+            const double partial = 2.0 * (double)pr * row_bytes / tile_bytes / grid_cap;
+            const double est = makespan(false, grid_cap) + makespan(true, grid_cap_umma) + partial;
+            if (best < 0.0 || est < best) {
+                best = est;
+                best_chunk = ct;
+            }
+        }
+        if (best_chunk < 0) return SPORK_ERR_INVALID;
+        chunk_tiles = best_chunk;
+        if (!split(chunk_tiles, &part_rows, &n_items)) return SPORK_ERR_INVALID;
     }
     for (QRowDesc &d : qd) {
         if (d.pre_base >= 0) {
@@ -290,7 +354,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         }
     }
     const int grid = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
-    const int grid_umma = (int)std::min<size_t>(items_umma.size(), (size_t)attn_umma_grid(c));
+    const int grid_umma = (int)std::min<size_t>(items_umma.size(), (size_t)grid_cap_umma);
     std::vector<int32_t> cta_ptr, cta_ptr_umma;
     if (mma) {
         schedule(items, grid, cta_ptr);

@@ -123,7 +123,7 @@ struct spork_ctx {
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
     int timing = 0;
-    int umma_min_rows = 33;       // segments with at least this many rows take the tcgen05 path
+    int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;
 };

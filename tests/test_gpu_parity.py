@@ -135,6 +135,31 @@ def test_small_bf16_decode(cfg, path):
     assert np.array_equal(out1.cpu().numpy(), out_b.cpu().numpy())
 
 
+@pytest.mark.parametrize("path", ["tcgen05", "mma.sync"])
+@pytest.mark.parametrize("frac,scale", [(0.01, 8.0), (0.05, 16.0), (0.3, 4.0)])
+def test_outlier_keys_running_max_jumps(frac, scale, path):
+    """Attention-sink outliers (BASELINE.json config 3): the running row max jumps by far more than
+    the tcgen05 kernel's lazy-rescale threshold in the middle of an item, so O is rescaled in TMEM;
+    near-one-hot rows must still come out within tolerance."""
+    cfg = synth.CFG3.scaled(n_groups=2, prefix_len=1040, suffix_lo=1, suffix_hi=150,
+                            outlier_frac=frac, outlier_scale=scale)
+    wl, orc, spk, ids = _build_both(cfg)
+    _set_path(spk, path)
+    q = wl.q_all()
+    out_ref, lse_ref = orc.decode(ids, q)
+    out, lse = spk.decode_attn(wl.group_indptr(), ids, q)
+    check_attn(out, lse, out_ref, lse_ref, "bf16", f"outliers {frac} x{scale}")
+    # the same through verify (k = 3 drafts per sequence, causal tail)
+    kk = np.full(cfg.n_seqs, 3)
+    cfgv = cfg.scaled(k_draft=3)
+    wl, orc, spk, ids = _build_both(cfgv, kk)
+    _set_path(spk, path)
+    q, qi = wl.q_all(), wl.q_indptr()
+    out_ref, lse_ref = orc.verify(ids, qi, q)
+    out, lse = spk.verify_attn(wl.group_indptr(), ids, qi, q)
+    check_attn(out, lse, out_ref, lse_ref, "bf16", f"verify outliers {frac} x{scale}")
+
+
 def test_small_fp32_generic_paths():
     # fp32 D = 128 and bf16 D = 64 go through the simt kernel
     for cfg in (synth.CFG1.scaled(D=128, Hq=8, Hkv=2, prefix_len=200, suffix_hi=70),
