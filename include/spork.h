@@ -204,7 +204,9 @@ typedef struct spork_plan_info {
     int64_t naive_tokens;   /* sum_members len                                      */
     int64_t partial_rows;   /* rows of split-KV workspace written                   */
     int32_t launches;       /* kernels launched by the last attention call          */
-    int32_t n_umma_items;   /* of n_items, those run by the tcgen05 kernel          */
+    int32_t n_umma_items;   /* of n_items, those run by the tcgen05 kernels         */
+    int32_t n_two_pipe_items; /* of those, items of <= 256 rows on the two-pipe variant */
+    int32_t reserved;
 } spork_plan_info;
 int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
 /* kernels launched by the last state call (append / fork / release / truncate) */
@@ -229,6 +231,14 @@ int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
  * cached plan.  SPORK_ERR_INVALID on a null context.
  */
 int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
+/*
+ * Tuning knob: allow (default) or forbid the two-pipe variant of the tcgen05 kernel.  Allowed:
+ * a tensor-path segment of more than 128 rows (verify: drafts x group members x GQA heads) is cut
+ * into row blocks of 256 and run by CTAs with two softmax pipes that share one stream of K/V
+ * tiles (one CTA per SM).  Forbidden: row blocks of 128 on the one-pipe kernel, each re-reading
+ * the K/V tiles through L2.  Results do not depend on it beyond rounding.  Invalidates the plan.
+ */
+int spork_set_two_pipe(spork_ctx *ctx, int enable);
 
 const char *spork_strerror(int code);
 

@@ -16,15 +16,21 @@ static int attn_common(spork_ctx *c, int n_groups, const int32_t *group_indptr, 
     if (P.info.kernel == 0) {
         rc = launch_attn_simt(c, q, st);
     } else {
-        // many-row items on the tcgen05 kernel first (the long shared-prefix streams), then the
-        // few-row items on the mma.sync kernel, which is allowed to start while the first drains
-        rc = launch_attn_umma(c, q, st);
-        if (rc == SPORK_OK) rc = launch_attn_mma(c, q, st);
+        // longest streams first: the two-pipe tcgen05 kernel (items of > 128 rows), the one-pipe
+        // tcgen05 kernel, then whatever the planner left to the mma.sync kernel.  A later kernel is
+        // launched programmatically: it may start while the earlier one drains, and does not
+        // complete before it (griddepcontrol.wait at its end), so the merge sees all partials.
+        bool prev = false;
+        rc = launch_attn_umma(c, q, 2, false, st);
+        prev = P.n_items_umma2 > 0;
+        if (rc == SPORK_OK) rc = launch_attn_umma(c, q, 1, prev, st);
+        prev = prev || P.n_items_umma > 0;
+        if (rc == SPORK_OK) rc = launch_attn_mma(c, q, prev, st);
     }
     if (rc != SPORK_OK) return rc;
     if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[1], st));
     if (P.info.kernel == 0) P.info.grid = P.n_items;
-    if (P.info.kernel == 2) P.info.grid = P.grid_umma;
+    if (P.info.kernel == 2) P.info.grid = P.grid_umma2 > 0 ? P.grid_umma2 : P.grid_umma;
     rc = launch_merge(c, out, lse, st);
     if (rc != SPORK_OK) return rc;
     if (c->timing) {
@@ -113,6 +119,13 @@ extern "C" int spork_last_kernel_ms(spork_ctx *c, float *attn_ms, float *merge_m
 extern "C" int spork_set_tensor_path_min_rows(spork_ctx *c, int min_rows) {
     if (!c) return SPORK_ERR_INVALID;
     c->umma_min_rows = min_rows;
+    c->plan.valid = false;
+    return SPORK_OK;
+}
+
+extern "C" int spork_set_two_pipe(spork_ctx *c, int enable) {
+    if (!c) return SPORK_ERR_INVALID;
+    c->two_pipe = enable ? 1 : 0;
     c->plan.valid = false;
     return SPORK_OK;
 }

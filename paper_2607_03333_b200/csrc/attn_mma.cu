@@ -446,7 +446,7 @@ namespace spork {
 
 int attn_mma_grid(spork_ctx *c) { return c->num_sms * CTAS_PER_SM; }
 
-int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st) {
+int launch_attn_mma(spork_ctx *c, const void *q, bool programmatic, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_items == 0) return SPORK_OK;
     static bool attr_set = false;
@@ -479,7 +479,7 @@ int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st) {
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = P.n_items_umma > 0 ? 1 : 0;   // overlap the tail of the tcgen05 kernel
+    cfg.numAttrs = programmatic ? 1 : 0;   // overlap the tail of the tcgen05 kernel
     SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_mma_kernel, p));
     c->last_launches++;
     c->plan.info.grid = grid;

@@ -9,6 +9,7 @@
 #include <math.h>
 
 #include "spork_internal.h"
+#include "merge.cuh"
 
 using namespace spork;
 
@@ -150,65 +151,10 @@ __global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__
                                                     float *__restrict__ out, float *__restrict__ lse) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= n_qrows * Hq) return;
-    const int qrow = w / Hq, h = w % Hq, kvh = h / G, j = h % G;
+    const int qrow = w / Hq, h = w % Hq;
     const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
-    const int pre0 = d.pre_base + kvh * d.pre_nq * G + d.pre_qi * G + j;
-    const int suf0 = d.suf_base + kvh * d.suf_nq * G + d.suf_qi * G + j;
-    const int n = d.pre_nsplit + d.suf_nsplit;
-    auto part = [&](int s) -> size_t {
-        return s < d.pre_nsplit ? (size_t)pre0 + (size_t)s * d.pre_stride
-                                : (size_t)suf0 + (size_t)(s - d.pre_nsplit) * d.suf_stride;
-    };
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    float M = -INFINITY;
-    for (int s = lane; s < n; s += 32) M = fmaxf(M, ws_lse[part(s)]);
-    M = warp_max(M);
-    const int nv = D >> 2;                        // float4 per row (<= 64)
-    float4 *o = reinterpret_cast<float4 *>(out + (size_t)w * D);
-    if (M == -INFINITY) {
-        for (int c = lane; c < nv; c += 32) o[c] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (lane == 0) lse[w] = -INFINITY;
-        return;
-    }
-    float4 acc[NI];
-#pragma unroll
-    for (int i = 0; i < NI; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    float W = 0.f;
-    for (int s0 = 0; s0 < n; s0 += 32) {
-        const int nb = min(32, n - s0);
-        const float wl = lane < nb ? expf(ws_lse[part(s0 + lane)] - M) : 0.f;   // weight of split s0+lane
-        for (int b0 = 0; b0 < nb; b0 += 8) {
-            float4 v[NI][8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(min(s0 + b0 + u, n - 1)) * D);
-#pragma unroll
-                for (int i = 0; i < NI; ++i) {
-                    const int c = lane + 32 * i;
-                    v[i][u] = c < nv ? po[c] : make_float4(0.f, 0.f, 0.f, 0.f);
-                }
-            }
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const float ws = __shfl_sync(0xffffffffu, wl, (b0 + u) & 31);   // 0 beyond nb
-                W += ws;
-#pragma unroll
-                for (int i = 0; i < NI; ++i) {
-                    acc[i].x = fmaf(ws, v[i][u].x, acc[i].x);
-                    acc[i].y = fmaf(ws, v[i][u].y, acc[i].y);
-                    acc[i].z = fmaf(ws, v[i][u].z, acc[i].z);
-                    acc[i].w = fmaf(ws, v[i][u].w, acc[i].w);
-                }
-            }
-        }
-    }
-    const float inv = 1.f / W;
-#pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        const int c = lane + 32 * i;
-        if (c < nv) o[c] = make_float4(acc[i].x * inv, acc[i].y * inv, acc[i].z * inv, acc[i].w * inv);
-    }
-    if (lane == 0) lse[w] = M + logf(W);
+    merge_row<NI>(d, h / G, h % G, G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
 }
 
 }  // namespace

@@ -31,17 +31,40 @@ constexpr int TILE_PAGES = 4;
 constexpr int TILE_TOKENS = TILE_PAGES * PS;          // 64
 constexpr int HEAD_BLOCK = PS * D * 2;                // 4096 B: one (page, kv head) block
 constexpr int SLOT_BYTES = TILE_PAGES * HEAD_BLOCK;   // 16 KiB: a K tile or a V tile
-constexpr int NSLOT = 5;
-constexpr int Q_BYTES = 128 * D * 2;                  // 32 KiB
+constexpr int Q_BYTES = 128 * D * 2;                  // 32 KiB: the 128 rows of one pipe
 constexpr int Q_HALF = Q_BYTES / 2;                   // dims [64, 128) start here
-constexpr int N_THREADS = 192;
-constexpr int CTAS_PER_SM = 2;
-constexpr int TMEM_COLS = 256;                        // O: [0,128)  S/P buffer b: [128 + 64 b, +64)
-constexpr int BAR_OFF = Q_BYTES + NSLOT * SLOT_BYTES;
-constexpr int SMEM_BYTES = BAR_OFF + 256;
+constexpr int PIPE_COLS = 256;                        // TMEM columns of one pipe: O [0,128), S/P buffer b [128 + 64 b, +64)
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 constexpr float RESCALE_THRESHOLD = 8.f;              // log2 units
+
+// NP = number of softmax pipes of a CTA = row blocks of 128 it runs against ONE stream of K/V:
+//   NP = 1: items of <= 128 rows, 2 CTAs per SM, 5-slot ring each
+//   NP = 2: items of <= 256 rows (verify with many drafts), 1 CTA per SM, 10-slot ring; every
+//           K/V tile is fetched once for both row blocks
+template <int NP>
+struct Cfg {
+    static constexpr int NSLOT = NP == 1 ? 5 : 10;
+    static constexpr int N_SOFTMAX = NP * 128;
+    static constexpr int N_THREADS = 64 + N_SOFTMAX;
+    static constexpr int CTAS_PER_SM = NP == 1 ? 2 : 1;
+    static constexpr int TMEM_COLS = NP * PIPE_COLS;
+    static constexpr int RING_OFF = NP * Q_BYTES;
+    static constexpr int BAR_OFF = RING_OFF + NSLOT * SLOT_BYTES;
+    // barrier slots (8 bytes each) from BAR_OFF
+    static constexpr int B_FULL = 0;                  // [NSLOT] bulk copies landed
+    static constexpr int B_EMPTY = NSLOT;             // [NSLOT] MMAs reading the slot completed
+    static constexpr int B_PIPE = 2 * NSLOT;          // per pipe: 7 barriers, see P_*
+    static constexpr int B_QFULL = B_PIPE + 7 * NP;   // Q staged
+    static constexpr int B_COUNT = B_QFULL + 1;
+    static constexpr int SMEM_BYTES = BAR_OFF + 8 * B_COUNT + 16;
+};
+enum : int {
+    P_SFULL = 0,    // [2] S(b) complete
+    P_PFULL = 2,    // [2] P(b) written (4 softmax warps)
+    P_PVDONE = 4,   // [2] P V of a tile with parity b complete
+    P_OFREE = 6     // epilogue finished reading O
+};
 
 struct UParams {
     const WorkItem *items;
@@ -54,50 +77,44 @@ struct UParams {
     float *ws_o, *ws_lse;
 };
 
-// barrier slots (8 bytes each) from BAR_OFF
-enum : int {
-    B_FULL = 0,                 // [NSLOT] bulk copies landed
-    B_EMPTY = NSLOT,            // [NSLOT] MMAs reading the slot completed
-    B_SFULL = 2 * NSLOT,        // [2] S(b) complete
-    B_PFULL = 2 * NSLOT + 2,    // [2] P(b) written (4 softmax warps)
-    B_PVDONE = 2 * NSLOT + 4,   // [2] P V of a tile with parity b complete
-    B_QFULL = 2 * NSLOT + 6,    // Q staged
-    B_OFREE = 2 * NSLOT + 7,    // epilogue finished reading O
-    B_COUNT = 2 * NSLOT + 8
-};
-
-__global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const UParams P) {
+template <int NP>
+__global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn_umma_kernel(const UParams P) {
+    using C = Cfg<NP>;
+    constexpr int NSLOT = C::NSLOT;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
-    const uint32_t bars = sbase + BAR_OFF;
-    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + BAR_OFF + 8 * B_COUNT);
+    const uint32_t ring = sbase + C::RING_OFF;
+    const uint32_t bars = sbase + C::BAR_OFF;
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + C::BAR_OFF + 8 * C::B_COUNT);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     auto bar = [&](int i) { return bars + 8u * (uint32_t)i; };
+    auto pbar = [&](int w, int i) { return bars + 8u * (uint32_t)(C::B_PIPE + 7 * w + i); };
 
     if (threadIdx.x == 0) {
         if (sbase & 1023u) __trap();   // the 128-byte swizzle is a function of the smem address
         for (int s = 0; s < NSLOT; ++s) {
-            mbar_init(bar(B_FULL + s), 1);
-            mbar_init(bar(B_EMPTY + s), 1);
+            mbar_init(bar(C::B_FULL + s), 1);
+            mbar_init(bar(C::B_EMPTY + s), 1);
         }
-        for (int b = 0; b < 2; ++b) {
-            mbar_init(bar(B_SFULL + b), 1);
-            mbar_init(bar(B_PFULL + b), 4);
-            mbar_init(bar(B_PVDONE + b), 1);
+        for (int w = 0; w < NP; ++w) {
+            for (int b = 0; b < 2; ++b) {
+                mbar_init(pbar(w, P_SFULL + b), 1);
+                mbar_init(pbar(w, P_PFULL + b), 4);
+                mbar_init(pbar(w, P_PVDONE + b), 1);
+            }
+            mbar_init(pbar(w, P_OFREE), 4);
         }
-        mbar_init(bar(B_QFULL), 1);
-        mbar_init(bar(B_OFREE), 4);
+        mbar_init(bar(C::B_QFULL), 1);
         mbar_fence_init();
     }
     if (warp == 1) {
-        tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+        tmem_alloc(smem_u32(tmem_slot), C::TMEM_COLS);
         tmem_relinquish();
     }
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tbase = *tmem_slot;
-    const uint32_t tO = tbase;
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     const int item_begin = P.cta_ptr[blockIdx.x], item_end = P.cta_ptr[blockIdx.x + 1];
@@ -131,94 +148,123 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
 #pragma unroll
                     for (int kv = 0; kv < 2; ++kv) {
                         const uint32_t slot = (ld + kv) % NSLOT, ph = ((ld + kv) / NSLOT) & 1;
-                        mbar_wait(bar(B_EMPTY + slot), ph ^ 1);
-                        mbar_expect_tx(bar(B_FULL + slot), (uint32_t)np * HEAD_BLOCK);
-                        const uint32_t dst = sbase + Q_BYTES + slot * SLOT_BYTES;
+                        mbar_wait(bar(C::B_EMPTY + slot), ph ^ 1);
+                        mbar_expect_tx(bar(C::B_FULL + slot), (uint32_t)np * HEAD_BLOCK);
+                        const uint32_t dst = ring + slot * SLOT_BYTES;
                         const uint8_t *pool = kv ? P.v_pool : P.k_pool;
 #pragma unroll
                         for (int p = 0; p < TILE_PAGES; ++p)
                             if (p < np)
                                 bulk_g2s(dst + p * HEAD_BLOCK, pool + (size_t)pg[p] * page_stride + head_off,
-                                         HEAD_BLOCK, bar(B_FULL + slot));
+                                         HEAD_BLOCK, bar(C::B_FULL + slot));
                     }
                 }
                 ld += 2;
             }
         }
     } else if (warp == 1) {
-        // ================================ MMA issuer (one thread) ================================
-        if (lane == 0) {
-            uint32_t g0 = 0;   // tiles issued before this item (global tile counter)
-            int j = 0;
-            for (int idx = item_begin; idx < item_end; ++idx, ++j) {
-                const WorkItem it = P.items[idx];
-                const int n_tok = it.tok1 - it.tok0;
-                const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
-                auto pages_of_tile = [&](int i) {
-                    return (min(TILE_TOKENS, n_tok - i * TILE_TOKENS) + PS - 1) / PS;
-                };
-                auto issue_s = [&](int i) {
-                    const uint32_t g = g0 + i, b = g & 1, ldk = 2 * g;
-                    const uint32_t slot = ldk % NSLOT, ph = (ldk / NSLOT) & 1;
-                    mbar_wait(bar(B_FULL + slot), ph);
-                    tc_fence_after();
-                    const uint32_t id = idesc_bf16(128, PS * pages_of_tile(i), 0, 0);
-                    const uint32_t ka = sbase + Q_BYTES + slot * SLOT_BYTES;
-                    const uint32_t tS = tbase + 128 + 64 * b;
+        // ================================ MMA issuer ================================
+        // The whole warp runs this loop in lockstep (waits, counters, descriptors stay warp-uniform);
+        // one elected lane issues the tcgen05 instructions of a step.
+        const uint64_t q_desc = smem_desc_sw128(sbase, 16, 1024);     // K-major, 8-row groups 1 KiB apart
+        const uint64_t k_desc = smem_desc_sw128(ring, 16, 2048);      // K-major, 8-token groups 2 KiB apart
+        const uint64_t v_desc = smem_desc_sw128(ring, 1024, 2048);    // MN-major: dim halves 1 KiB, 8-token groups 2 KiB
+        constexpr uint32_t ID_PV = idesc_bf16(128, D, 0, 1);
+        uint32_t gt = 0;            // tiles of all items so far: K of tile gt is load 2 gt, V is 2 gt + 1
+        uint32_t g0[NP];            // tiles pipe w has run (its S/P buffer and barrier phases)
+        int jw[NP];                 // items pipe w has run
 #pragma unroll
-                    for (int ks = 0; ks < 8; ++ks) {
-                        const uint64_t ad = smem_desc_sw128(sbase + (ks >> 2) * Q_HALF + (ks & 3) * 32, 16, 1024);
-                        const uint64_t bd = smem_desc_sw128(ka + (ks >> 2) * 1024 + (ks & 3) * 32, 16, 2048);
-                        mma_ss(tS, ad, bd, id, ks > 0);
-                    }
-                    mma_commit(bar(B_EMPTY + slot));
-                    mma_commit(bar(B_SFULL + b));
-                };
-                mbar_wait(bar(B_QFULL), j & 1);
+        for (int w = 0; w < NP; ++w) { g0[w] = 0; jw[w] = 0; }
+        int j = 0;
+        for (int idx = item_begin; idx < item_end; ++idx, ++j) {
+            const WorkItem it = P.items[idx];
+            const int n_tok = it.tok1 - it.tok0;
+            const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
+            const int npipe = (NP > 1 && it.nrows > 128) ? 2 : 1;   // pipe 1 sits idle on a <= 128-row item
+            auto pages_of_tile = [&](int i) {
+                return (min(TILE_TOKENS, n_tok - i * TILE_TOKENS) + PS - 1) / PS;
+            };
+            auto issue_s = [&](int i) {
+                const uint32_t ldk = 2 * (gt + i);
+                const uint32_t slot = ldk % NSLOT, ph = (ldk / NSLOT) & 1;
+                mbar_wait(bar(C::B_FULL + slot), ph);
                 tc_fence_after();
-                issue_s(0);
-                for (int i = 0; i < n_tiles; ++i) {
-                    if (i + 1 < n_tiles) issue_s(i + 1);
-                    const uint32_t g = g0 + i, b = g & 1, ldv = 2 * g + 1;
-                    const uint32_t slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
-                    mbar_wait(bar(B_PFULL + b), (g >> 1) & 1);
-                    mbar_wait(bar(B_FULL + slot), ph);
-                    if (i == 0 && j > 0) mbar_wait(bar(B_OFREE), (j - 1) & 1);
-                    tc_fence_after();
-                    const uint32_t id = idesc_bf16(128, D, 0, 1);
-                    const uint32_t va = sbase + Q_BYTES + slot * SLOT_BYTES;
-                    const uint32_t tP = tbase + 128 + 64 * b;
-                    const int nvp = pages_of_tile(i);
+                const uint32_t id = idesc_bf16(128, PS * pages_of_tile(i), 0, 0);
+                const uint64_t kd = smem_desc_advance(k_desc, slot * SLOT_BYTES);
+                if (elect_one()) {
 #pragma unroll
-                    for (int pg = 0; pg < TILE_PAGES; ++pg)
-                        if (pg < nvp) {
-                            const uint64_t bd = smem_desc_sw128(va + pg * HEAD_BLOCK, 1024, 2048);
-                            mma_ts(tO, tP + pg * 8, bd, id, (i > 0) || (pg > 0));
+                    for (int w = 0; w < NP; ++w) {
+                        if (w < npipe) {
+                            const uint32_t b = (g0[w] + i) & 1;
+                            const uint32_t tS = tbase + w * PIPE_COLS + 128 + 64 * b;
+#pragma unroll
+                            for (int ks = 0; ks < 8; ++ks)
+                                mma_ss(tS, smem_desc_advance(q_desc, w * Q_BYTES + (ks >> 2) * Q_HALF + (ks & 3) * 32),
+                                       smem_desc_advance(kd, (ks >> 2) * 1024 + (ks & 3) * 32), id, ks > 0);
+                            mma_commit(pbar(w, P_SFULL + b));
                         }
-                    mma_commit(bar(B_EMPTY + slot));
-                    mma_commit(bar(B_PVDONE + b));
+                    }
+                    mma_commit(bar(C::B_EMPTY + slot));
                 }
-                g0 += n_tiles;
+                __syncwarp();
+            };
+            mbar_wait(bar(C::B_QFULL), j & 1);
+            tc_fence_after();
+            issue_s(0);
+            for (int i = 0; i < n_tiles; ++i) {
+                if (i + 1 < n_tiles) issue_s(i + 1);
+                const uint32_t ldv = 2 * (gt + i) + 1;
+                const uint32_t slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
+                const uint64_t vd = smem_desc_advance(v_desc, slot * SLOT_BYTES);
+                const int nvp = pages_of_tile(i);
+#pragma unroll
+                for (int w = 0; w < NP; ++w) {
+                    if (w < npipe) {
+                        const uint32_t g = g0[w] + i, b = g & 1;
+                        mbar_wait(pbar(w, P_PFULL + b), (g >> 1) & 1);
+                        if (w == 0) mbar_wait(bar(C::B_FULL + slot), ph);
+                        if (i == 0 && jw[w] > 0) mbar_wait(pbar(w, P_OFREE), (jw[w] - 1) & 1);
+                        tc_fence_after();
+                        const uint32_t tO = tbase + w * PIPE_COLS;
+                        const uint32_t tP = tO + 128 + 64 * b;
+                        if (elect_one()) {
+                            mma_ts(tO, tP, vd, ID_PV, i > 0);
+#pragma unroll
+                            for (int pg = 1; pg < TILE_PAGES; ++pg)
+                                if (pg < nvp) mma_ts(tO, tP + pg * 8, smem_desc_advance(vd, pg * HEAD_BLOCK), ID_PV, 1);
+                            mma_commit(pbar(w, P_PVDONE + b));
+                            if (w == npipe - 1) mma_commit(bar(C::B_EMPTY + slot));
+                        }
+                        __syncwarp();
+                    }
+                }
             }
+            gt += n_tiles;
+#pragma unroll
+            for (int w = 0; w < NP; ++w)
+                if (w < npipe) { g0[w] += n_tiles; jw[w]++; }
         }
-        __syncwarp();
     } else {
         // ================================ softmax warps ================================
+        const int w = NP > 1 ? (warp - 2) >> 2 : 0;    // pipe: rows [128 w, 128 w + 128) of the item
         const int lg = warp & 3;                       // TMEM lane group this warp may access
-        const int r = lg * 32 + lane;                  // query row of the item owned by this thread
+        const int r = w * 128 + lg * 32 + lane;        // query row of the item owned by this thread
         const uint32_t lane_addr = (uint32_t)(lg * 32) << 16;
-        const int st = threadIdx.x - 64;               // 0..127 among the softmax threads
-        uint32_t g0 = 0;
+        const uint32_t tO = tbase + w * PIPE_COLS;
+        const int st = threadIdx.x - 64;               // 0 .. N_SOFTMAX-1 among the softmax threads
+        uint32_t g0 = 0, gt = 0;                       // tiles this pipe has run / tiles of all items so far
         for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = P.items[idx];
             const int n_tok = it.tok1 - it.tok0;
             const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
             // ---- Q rows -> smem (K-major, 128-byte swizzle); rows beyond nrows are zero ----
             {
+                // each pipe stages its own 128 rows: its previous Q image is free once ITS last P V of the
+                // previous item has completed, whatever the other pipe is still doing
                 const int c = st & 15;                 // 16-byte chunk of the row
 #pragma unroll 4
                 for (int k = 0; k < 16; ++k) {
-                    const int row = (st >> 4) + 8 * k;
+                    const int row = w * 128 + ((st & 127) >> 4) + 8 * k;
                     uint4 v = make_uint4(0, 0, 0, 0);
                     if (row < it.nrows) {
                         const int lr = it.rb0 + row;
@@ -226,39 +272,45 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                             P.q + ((size_t)(it.qrow0 + lr / P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D + c * 8;
                         v = *reinterpret_cast<const uint4 *>(src);
                     }
-                    const int off = (c >> 3) * Q_HALF + (row >> 3) * 1024 + (row & 7) * 128 +
-                                    (((c & 7) ^ (row & 7)) << 4);
+                    const int rp = row & 127;          // row inside its pipe's 32 KiB image
+                    const int off = (row >> 7) * Q_BYTES + (c >> 3) * Q_HALF + (rp >> 3) * 1024 + (rp & 7) * 128 +
+                                    (((c & 7) ^ (rp & 7)) << 4);
                     *reinterpret_cast<uint4 *>(smem + off) = v;
                 }
                 fence_async_smem();
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (st == 0) mbar_arrive(bar(B_QFULL));
+                asm volatile("bar.sync 1, %0;" ::"n"(C::N_SOFTMAX) : "memory");
+                if (st == 0) mbar_arrive(bar(C::B_QFULL));
+            }
+            if (NP > 1 && w * 128 >= it.nrows) {       // this pipe sits the item out (the MMA thread knows)
+                gt += n_tiles;
+                continue;
             }
             const int lim_r = it.lim0 + (it.rb0 + r) / P.G;
-            const int min_lim = it.lim0 + it.rb0 / P.G;
+            const int min_lim = it.lim0 + (it.rb0 + w * 128) / P.G;
             float m_used = -INFINITY, l = 0.f, lr = 0.f;   // l: exact row sum (lse); lr: sum of the bf16 weights
 
-            if (lg * 32 >= it.nrows) {
+            if (w * 128 + lg * 32 >= it.nrows) {
                 // none of this warp's 32 rows exists (few-row item): only keep the barriers moving;
                 // whatever S/P/O hold in these lanes never leaves TMEM
                 for (int i = 0; i < n_tiles; ++i) {
                     const uint32_t g = g0 + i, b = g & 1;
-                    mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
-                    if (lane == 0) mbar_arrive(bar(B_PFULL + b));
+                    mbar_wait(pbar(w, P_SFULL + b), (g >> 1) & 1);
+                    if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
                     __syncwarp();
                 }
                 const uint32_t gl = g0 + n_tiles - 1;
-                mbar_wait(bar(B_PVDONE + (gl & 1)), (gl >> 1) & 1);
-                if (lane == 0) mbar_arrive(bar(B_OFREE));
+                mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
                 __syncwarp();
                 g0 += n_tiles;
+                gt += n_tiles;
                 continue;
             }
 
             for (int i = 0; i < n_tiles; ++i) {
                 const uint32_t g = g0 + i, b = g & 1;
-                const uint32_t tS = tbase + 128 + 64 * b + lane_addr;
-                mbar_wait(bar(B_SFULL + b), (g >> 1) & 1);
+                const uint32_t tS = tO + 128 + 64 * b + lane_addr;
+                mbar_wait(pbar(w, P_SFULL + b), (g >> 1) & 1);
                 tc_fence_after();
                 uint32_t s0[32], s1[32];
                 tmem_ld32(tS, s0);
@@ -287,7 +339,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                     lr *= alpha;
                     if (i > 0) {
                         // O holds tiles [0, i): wait for P V(i - 1), rescale this thread's row
-                        mbar_wait(bar(B_PVDONE + ((g - 1) & 1)), ((g - 1) >> 1) & 1);
+                        mbar_wait(pbar(w, P_PVDONE + ((g - 1) & 1)), ((g - 1) >> 1) & 1);
                         tc_fence_after();
 #pragma unroll 1
                         for (int cb = 0; cb < 4; ++cb) {
@@ -326,14 +378,15 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                 lr += rs0 + rs1;
                 tmem_st32(tS, p);
                 tmem_wait_st();
-                if ((nv & (PS - 1)) && lg == 0) {
+                if ((nv & (PS - 1)) && w == 0 && lg == 0) {
                     // the last staged page is partially filled: its tail rows hold whatever the pool
-                    // held (possibly NaN patterns).  P is 0 there; make V 0 as well (the warp of rows
-                    // 0..31 does it: it is active in every item).
-                    const uint32_t ldv = 2 * g + 1, slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
-                    mbar_wait(bar(B_FULL + slot), ph);
+                    // held (possibly NaN patterns).  P is 0 there; make V 0 as well.  The warp of rows
+                    // 0..31 does it (active in every item); the MMA thread issues pipe 0's P V, which
+                    // waits for this warp, before any other pipe's.
+                    const uint32_t ldv = 2 * (gt + i) + 1, slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
+                    mbar_wait(bar(C::B_FULL + slot), ph);
                     const int nvp = (nv + PS - 1) / PS;
-                    uint8_t *vpage = smem + Q_BYTES + slot * SLOT_BYTES + (nvp - 1) * HEAD_BLOCK;
+                    uint8_t *vpage = smem + C::RING_OFF + slot * SLOT_BYTES + (nvp - 1) * HEAD_BLOCK;
                     const int r_first = nv & (PS - 1);
                     for (int e = lane; e < (PS - r_first) * 16; e += 32) {
                         const int rr = r_first + (e >> 4), cc = e & 15;
@@ -343,13 +396,13 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_PFULL + b));
+                if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
             }
 
             // ---- epilogue: O / l -> partial rows ------------------------------------------------
             {
                 const uint32_t gl = g0 + n_tiles - 1;
-                mbar_wait(bar(B_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
                 tc_fence_after();
                 const float inv = lr > 0.f ? 1.f / lr : 0.f;
                 float *dst = P.ws_o + (size_t)(it.part_base + r) * D;
@@ -370,9 +423,10 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
                     P.ws_lse[it.part_base + r] = l > 0.f ? (m_used + log2f(l)) * LN2 : -INFINITY;
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(B_OFREE));
+                if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
             }
             g0 += n_tiles;
+            gt += n_tiles;
         }
     }
 
@@ -381,28 +435,55 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_umma_kernel(const
     __syncthreads();
     if (warp == 1) {
         tc_fence_after();
-        tmem_dealloc(tbase, TMEM_COLS);
+        tmem_dealloc(tbase, C::TMEM_COLS);
     }
+    // When launched programmatically behind another attention kernel this grid may start before
+    // that one has finished; do not complete before it has, so that merge_kernel (which waits for
+    // the LAST attention grid) sees every kernel's partials.  A no-op for a normal launch.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 }  // namespace
 
 namespace spork {
 
-int attn_umma_grid(spork_ctx *c) { return c->num_sms * CTAS_PER_SM; }
+int attn_umma_grid(spork_ctx *c, int np) {
+    return c->num_sms * (np == 1 ? Cfg<1>::CTAS_PER_SM : Cfg<2>::CTAS_PER_SM);
+}
 
-int launch_attn_umma(spork_ctx *c, const void *q, cudaStream_t st) {
-    const Plan &P = c->plan;
-    if (P.n_items_umma == 0) return SPORK_OK;
+template <int NP>
+static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        SMEM_BYTES));
+        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg<NP>::SMEM_BYTES));
         attr_set = true;
     }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(Cfg<NP>::N_THREADS);
+    cfg.dynamicSmemBytes = Cfg<NP>::SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = programmatic ? 1 : 0;   // may start while the previous attention kernel drains
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP>, p));
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
+// np = 2: the <= 256-row items (launched first), np = 1: the <= 128-row items
+int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st) {
+    const Plan &P = c->plan;
+    const int n = np == 2 ? P.n_items_umma2 : P.n_items_umma;
+    if (n == 0) return SPORK_OK;
     UParams p;
-    p.items = (const WorkItem *)P.items.p + P.n_items;        // the tensor-path items follow the others
-    p.cta_ptr = (const int32_t *)P.cta_ptr.p + (P.grid + 1);
+    // item lists: [mma.sync][tcgen05 NP=1][tcgen05 NP=2]; cta_ptr arrays in the same order
+    p.items = (const WorkItem *)P.items.p + P.n_items + (np == 2 ? P.n_items_umma : 0);
+    p.cta_ptr = (const int32_t *)P.cta_ptr.p + (P.grid + 1) + (np == 2 ? P.grid_umma + 1 : 0);
     p.q = (const uint16_t *)q;
     p.k_pool = (const uint8_t *)c->k_pool;
     p.v_pool = (const uint8_t *)c->v_pool;
@@ -414,10 +495,8 @@ int launch_attn_umma(spork_ctx *c, const void *q, cudaStream_t st) {
     p.scale_log2 = c->cfg.scale * LOG2E;
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
-    attn_umma_kernel<<<P.grid_umma, N_THREADS, SMEM_BYTES, st>>>(p);
-    c->last_launches++;
-    SPORK_CUDA(cudaGetLastError());
-    return SPORK_OK;
+    return np == 2 ? launch_np<2>(c, p, P.grid_umma2, programmatic, st)
+                   : launch_np<1>(c, p, P.grid_umma, programmatic, st);
 }
 
 }  // namespace spork

@@ -1,0 +1,87 @@
+// libspork: LSE-weighted combination of one (q row, q head)'s partials by one warp.
+//   M = max lse_s, w_s = exp(lse_s - M), out = sum w_s o_s / sum w_s, lse = M + ln sum w_s
+// An empty partial has lse = -inf and weight 0; no partial at all: out = 0, lse = -inf.
+// The partials were written by the attention kernel(s) just before and sit in L2: every
+// partial is read once, with ld.global.cg.
+#pragma once
+
+#include <math.h>
+
+#include "spork_internal.h"
+
+namespace spork {
+
+__device__ __forceinline__ float merge_warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
+// every load of a batch in flight before the first use (pure L2 latency otherwise).
+template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
+__device__ __forceinline__ void merge_row(const QRowDesc &d, int kvh, int j, int G, int D,
+                                          const float *ws_o, const float *ws_lse, float *out_row,
+                                          float *lse_out, int lane) {
+    const int pre0 = d.pre_base + kvh * d.pre_nq * G + d.pre_qi * G + j;
+    const int suf0 = d.suf_base + kvh * d.suf_nq * G + d.suf_qi * G + j;
+    const int n = d.pre_nsplit + d.suf_nsplit;
+    auto part = [&](int s) -> size_t {
+        return s < d.pre_nsplit ? (size_t)pre0 + (size_t)s * d.pre_stride
+                                : (size_t)suf0 + (size_t)(s - d.pre_nsplit) * d.suf_stride;
+    };
+    const float lse_mine = lane < n ? __ldcg(ws_lse + part(lane)) : -INFINITY;   // split `lane`
+    float M = lse_mine;
+    for (int s = lane + 32; s < n; s += 32) M = fmaxf(M, __ldcg(ws_lse + part(s)));
+    M = merge_warp_max(M);
+    const int nv = D >> 2;                        // float4 per row (<= 64)
+    float4 *o = reinterpret_cast<float4 *>(out_row);
+    if (M == -INFINITY) {
+        for (int c = lane; c < nv; c += 32) o[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (lane == 0) *lse_out = -INFINITY;
+        return;
+    }
+    float4 acc[NI];
+#pragma unroll
+    for (int i = 0; i < NI; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    float W = 0.f;
+    for (int s0 = 0; s0 < n; s0 += 32) {
+        const int nb = min(32, n - s0);
+        const float wl = lane < nb ? expf((s0 == 0 ? lse_mine : __ldcg(ws_lse + part(s0 + lane))) - M)
+                                   : 0.f;                                   // weight of split s0+lane
+        for (int b0 = 0; b0 < nb; b0 += 8) {
+            float4 v[NI][8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const bool have = b0 + u < nb;          // no load beyond the last split
+                const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(have ? s0 + b0 + u : 0) * D);
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int c = lane + 32 * i;
+                    v[i][u] = have && c < nv ? __ldcg(po + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float ws = __shfl_sync(0xffffffffu, wl, (b0 + u) & 31);   // 0 beyond nb
+                W += ws;
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    acc[i].x = fmaf(ws, v[i][u].x, acc[i].x);
+                    acc[i].y = fmaf(ws, v[i][u].y, acc[i].y);
+                    acc[i].z = fmaf(ws, v[i][u].z, acc[i].z);
+                    acc[i].w = fmaf(ws, v[i][u].w, acc[i].w);
+                }
+            }
+        }
+    }
+    const float inv = 1.f / W;
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        const int c = lane + 32 * i;
+        if (c < nv) o[c] = make_float4(acc[i].x * inv, acc[i].y * inv, acc[i].z * inv, acc[i].w * inv);
+    }
+    if (lane == 0) *lse_out = M + logf(W);
+}
+
+}  // namespace spork

@@ -6,9 +6,11 @@
 //   prefix segment  (one per group):  all members' rows x the shared pages, read once
 //   suffix segment  (one per member): that member's rows x its private tokens
 // Each segment is cut into equal chunks of whole 64-token tiles; one work item
-// per (chunk, kv head, row block).  Segments with many rows (>= umma_min_rows: the GQA
-// heads of a whole fork group, or a verify call's drafts) go to the tcgen05 kernel in
-// row blocks of <= 128; the others to the mma.sync kernel in row blocks of <= 64.
+// per (chunk, kv head, row block).  Segments with >= umma_min_rows rows (default: all) go
+// to the tcgen05 kernel: in row blocks of <= 128 (one softmax pipe per CTA), or, when a
+// segment has more than 128 rows (a verify call's drafts x group x GQA heads), in row
+// blocks of <= 256 to the two-pipe variant, which fetches each K/V tile once for both
+// halves.  The others go to the mma.sync kernel in row blocks of <= 64.
 // Each kernel's items are sorted longest first and statically scheduled onto its
 // persistent CTAs.
 #include <limits.h>
@@ -63,7 +65,7 @@ struct Segment {
     int lim0;
     int part_base, nsplit, chunk_tiles;
     bool prefix;
-    bool umma;
+    int kind;                   // 0: mma.sync / simt, 1: tcgen05 one pipe, 2: tcgen05 two pipes
     int row_block;
 };
 
@@ -193,7 +195,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         int pre_seg = -1;
         if (S > 0) {
             pre_seg = (int)segs.size();
-            segs.push_back({seq_ids[b], 0, S, gq0, gnq, INT_MAX / 2, 0, 0, 0, true, false, ROW_BLOCK});
+            segs.push_back({seq_ids[b], 0, S, gq0, gnq, INT_MAX / 2, 0, 0, 0, true, 0, ROW_BLOCK});
         }
         unique_tokens += S;
         for (int i = b; i < e; ++i) {
@@ -203,7 +205,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             int suf_seg = -1;
             if (L > S) {
                 suf_seg = (int)segs.size();
-                segs.push_back({seq_ids[i], S, L, q0, k, L - k, 0, 0, 0, false, false, ROW_BLOCK});
+                segs.push_back({seq_ids[i], S, L, q0, k, L - k, 0, 0, 0, false, 0, ROW_BLOCK});
             }
             unique_tokens += L - S;
             for (int j = 0; j < k; ++j) {
@@ -224,8 +226,9 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     const int grid_cap = mma ? attn_mma_grid(c) : c->num_sms * 4;
     int64_t total_cost = 0;
     for (Segment &s : segs) {
-        s.umma = mma && s.nq * G >= c->umma_min_rows;
-        s.row_block = s.umma ? ROW_BLOCK_UMMA : ROW_BLOCK;
+        const int rows = s.nq * G;
+        s.kind = !(mma && rows >= c->umma_min_rows) ? 0 : (rows > ROW_BLOCK_UMMA && c->two_pipe ? 2 : 1);
+        s.row_block = s.kind == 0 ? ROW_BLOCK : s.kind * ROW_BLOCK_UMMA;
         int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
         total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, s.row_block);
     }
@@ -234,7 +237,8 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     // costs its tiles plus a fixed part (Q staging, partial write-back); the partials are written
     // once and read once by the merge kernel, which all CTAs share.  Fewer, longer items cost less
     // overhead and less partial traffic; more, shorter items balance the persistent CTAs better.
-    const int grid_cap_umma = mma ? attn_umma_grid(c) : 0;
+    const int grid_cap_umma = mma ? attn_umma_grid(c, 1) : 0;
+    const int grid_cap_umma2 = mma ? attn_umma_grid(c, 2) : 0;
     auto split = [&](int chunk_tiles, int64_t *part_rows_out, size_t *n_items_out) -> bool {
         int64_t part_rows = 0;
         size_t n_items = 0;
@@ -252,15 +256,16 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         *n_items_out = n_items;
         return true;
     };
-    auto makespan = [&](bool umma, int grid) -> double {
+    auto makespan = [&](int kind, int grid) -> double {
         std::vector<float> cost;
         for (const Segment &s : segs) {
-            if (s.umma != umma) continue;
+            if (s.kind != kind) continue;
             const int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
             const int n_rb = ceil_div(s.nq * G, s.row_block);
             for (int sp = 0; sp < s.nsplit; ++sp) {
-                const float t = (float)std::min(s.chunk_tiles, tiles - sp * s.chunk_tiles) +
-                                (umma ? ITEM_FIXED_COST_UMMA : ITEM_FIXED_COST);
+                // a two-pipe CTA has the SM to itself: a tile takes it half the time of a one-pipe CTA
+                const float t = ((float)std::min(s.chunk_tiles, tiles - sp * s.chunk_tiles) +
+                                 (kind ? ITEM_FIXED_COST_UMMA : ITEM_FIXED_COST)) * (kind == 2 ? 0.5f : 1.f);
                 cost.insert(cost.end(), (size_t)Hkv * n_rb, t);
             }
         }
@@ -295,7 +300,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             size_t ni;
             if (!split(ct, &pr, &ni)) continue;
             const double partial = 2.0 * (double)pr * row_bytes / tile_bytes / grid_cap;
-            const double est = makespan(false, grid_cap) + makespan(true, grid_cap_umma) + partial;
+            const double est = makespan(0, grid_cap) + makespan(1, grid_cap_umma) + makespan(2, grid_cap_umma2) + partial;
             if (best < 0.0 || est < best) {
                 best = est;
                 best_chunk = ct;
@@ -327,12 +332,12 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     }
 
     // ---- items of the two kernels, each longest first and statically scheduled -----------------
-    std::vector<WorkItem> items, items_umma;
+    std::vector<WorkItem> items, items_umma, items_umma2;
     items.reserve(n_items);
     int n_prefix_items = 0;
     for (const Segment &s : segs) {
         const int rows = s.nq * G;
-        std::vector<WorkItem> &dst = s.umma ? items_umma : items;
+        std::vector<WorkItem> &dst = s.kind == 2 ? items_umma2 : (s.kind == 1 ? items_umma : items);
         for (int sp = 0; sp < s.nsplit; ++sp) {
             int t0 = s.tok0 + sp * s.chunk_tiles * TILE_TOKENS;
             int t1 = std::min(s.tok1, t0 + s.chunk_tiles * TILE_TOKENS);
@@ -355,20 +360,25 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     }
     const int grid = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
     const int grid_umma = (int)std::min<size_t>(items_umma.size(), (size_t)grid_cap_umma);
-    std::vector<int32_t> cta_ptr, cta_ptr_umma;
+    const int grid_umma2 = (int)std::min<size_t>(items_umma2.size(), (size_t)grid_cap_umma2);
+    std::vector<int32_t> cta_ptr, cta_ptr_umma, cta_ptr_umma2;
     if (mma) {
         schedule(items, grid, cta_ptr);
         schedule(items_umma, grid_umma, cta_ptr_umma);
+        schedule(items_umma2, grid_umma2, cta_ptr_umma2);
     } else {
         std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
             return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
         });
         cta_ptr.assign(grid + 1, 0);
         cta_ptr_umma.assign(1, 0);
+        cta_ptr_umma2.assign(1, 0);
     }
     const int n_items_mma = (int)items.size();
     items.insert(items.end(), items_umma.begin(), items_umma.end());
+    items.insert(items.end(), items_umma2.begin(), items_umma2.end());
     cta_ptr.insert(cta_ptr.end(), cta_ptr_umma.begin(), cta_ptr_umma.end());
+    cta_ptr.insert(cta_ptr.end(), cta_ptr_umma2.begin(), cta_ptr_umma2.end());
 
     // ---- upload (the previous plan's buffers may still be in use by queued kernels) -----------
     if (c->plan_ev_pending) {
@@ -402,9 +412,11 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     }
 
     P.n_items = n_items_mma;
-    P.n_items_umma = (int)items.size() - n_items_mma;
+    P.n_items_umma = (int)items_umma.size();
+    P.n_items_umma2 = (int)items_umma2.size();
     P.grid = grid;
     P.grid_umma = grid_umma;
+    P.grid_umma2 = grid_umma2;
     P.n_qrows = n_qrows;
     P.verify = verify;
     P.len_epoch = c->len_epoch;
@@ -413,11 +425,12 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     P.seq_ids.assign(seq_ids, seq_ids + n_seq);
     if (verify) P.q_indptr.assign(q_indptr, q_indptr + n_seq + 1); else P.q_indptr.clear();
     P.info = spork_plan_info{};
-    P.info.n_items = P.n_items + P.n_items_umma;
-    P.info.n_umma_items = P.n_items_umma;
+    P.info.n_items = P.n_items + P.n_items_umma + P.n_items_umma2;
+    P.info.n_umma_items = P.n_items_umma + P.n_items_umma2;
+    P.info.n_two_pipe_items = P.n_items_umma2;
     P.info.n_prefix_items = n_prefix_items;
     P.info.chunk_tokens = chunk_tiles * TILE_TOKENS;
-    P.info.kernel = !mma ? 0 : (P.n_items_umma == 0 ? 1 : (P.n_items == 0 ? 2 : 3));
+    P.info.kernel = !mma ? 0 : (P.info.n_umma_items == 0 ? 1 : (P.n_items == 0 ? 2 : 3));
     P.info.plan_cached = 0;
     P.info.unique_tokens = unique_tokens;
     P.info.naive_tokens = naive_tokens;

@@ -27,7 +27,7 @@ struct WorkItem {
     int32_t kvh;
     int32_t qrow0;
     int32_t rb0;
-    int32_t nrows;      // <= 64 (mma.sync / simt path), <= 128 (tcgen05 path)
+    int32_t nrows;      // <= 64 (mma.sync / simt path), <= 128 / 256 (tcgen05 kernel, one / two pipes)
     int32_t lim0;
     int32_t part_base;  // partial row index of logical row rb0
     int32_t pad[3];
@@ -71,12 +71,14 @@ struct Plan {
     std::vector<int32_t> shared_key_indptr, shared_key_ids;
     // device copies
     DevBuf items, qdesc;
-    // items = [n_items of the mma.sync / simt path][n_items_umma of the tcgen05 path];
-    // cta_ptr = int32[grid + 1] then int32[grid_umma + 1]: CTA b of a kernel runs items
-    // [cta_ptr[b], cta_ptr[b + 1]) of its own list
+    // items = [n_items of the mma.sync / simt path][n_items_umma of the tcgen05 kernel, <= 128 rows]
+    //         [n_items_umma2 of the two-pipe tcgen05 kernel, <= 256 rows];
+    // cta_ptr = int32[grid + 1], int32[grid_umma + 1], int32[grid_umma2 + 1]: CTA b of a kernel
+    // runs items [cta_ptr[b], cta_ptr[b + 1]) of its own list
     DevBuf cta_ptr;
     int n_items = 0, n_qrows = 0, grid = 0;
     int n_items_umma = 0, grid_umma = 0;
+    int n_items_umma2 = 0, grid_umma2 = 0;
     spork_plan_info info{};
 };
 
@@ -123,6 +125,7 @@ struct spork_ctx {
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
     int timing = 0;
+    int two_pipe = 1;             // segments of > 128 rows run on the two-pipe tcgen05 kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;
@@ -155,11 +158,11 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
 
 // attention launchers
 int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st);
-int launch_attn_mma(spork_ctx *c, const void *q, cudaStream_t st);
 int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st);
 int attn_mma_grid(spork_ctx *c);
-int launch_attn_umma(spork_ctx *c, const void *q, cudaStream_t st);
-int attn_umma_grid(spork_ctx *c);
+int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st);
+int attn_umma_grid(spork_ctx *c, int np);
+int launch_attn_mma(spork_ctx *c, const void *q, bool programmatic, cudaStream_t st);
 
 // Swizzled (page, kv head) block, bf16 with D % 64 == 0: the block is a run of 1 KiB
 // atoms of 8 token rows x 128 bytes (64 dims), ordered [row group r/8][dim half d/64];

@@ -115,6 +115,21 @@ __device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t saddr, uint32_t lbo
     d |= (uint64_t)2 << 61;
     return d;
 }
+// The descriptor of the same layout `bytes` further on (start addresses stay below 256 KiB, so the
+// 14-bit field never carries): the issuing thread builds a base descriptor once and adds offsets.
+__device__ __forceinline__ uint64_t smem_desc_advance(uint64_t desc, uint32_t bytes) {
+    return desc + (uint64_t)(bytes >> 4);
+}
+// one lane of a converged warp
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\t"
+        "elect.sync _|P, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t}"
+        : "=r"(pred));
+    return pred != 0;
+}
 // Instruction descriptor, kind::f16, bf16 x bf16 -> f32:
 //   [4,6) D format = 1 (f32)  [7,10) A format = 1 (bf16)  [10,13) B format = 1 (bf16)
 //   [15] A MN-major  [16] B MN-major  [17,23) N >> 3  [24,29) M >> 4

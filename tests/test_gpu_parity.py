@@ -93,17 +93,21 @@ SMALL_DECODE = [
 
 
 # planner knob: which segments run on the tcgen05 kernel (None = default threshold)
-PATHS = {"auto": None, "tcgen05": 1, "mma.sync": 1 << 20}
+PATHS = {"auto": None, "tcgen05": 1, "tcgen05-one-pipe": 1, "mma.sync": 1 << 20}
 
 
 def _set_path(spk, path):
     if PATHS[path] is not None:
         spk.set_tensor_path_min_rows(PATHS[path])
+    if path == "tcgen05-one-pipe":
+        spk.set_two_pipe(False)
 
 
 def _check_kernel(info, path):
-    if path == "tcgen05":
+    if path.startswith("tcgen05"):
         assert info["kernel"] == 2 and info["n_umma_items"] == info["n_items"]
+        if path == "tcgen05-one-pipe":
+            assert info["n_two_pipe_items"] == 0
     elif path == "mma.sync":
         assert info["kernel"] == 1 and info["n_umma_items"] == 0
     else:
@@ -149,9 +153,10 @@ def test_outlier_keys_running_max_jumps(frac, scale, path):
     out_ref, lse_ref = orc.decode(ids, q)
     out, lse = spk.decode_attn(wl.group_indptr(), ids, q)
     check_attn(out, lse, out_ref, lse_ref, "bf16", f"outliers {frac} x{scale}")
-    # the same through verify (k = 3 drafts per sequence, causal tail)
-    kk = np.full(cfg.n_seqs, 3)
-    cfgv = cfg.scaled(k_draft=3)
+    # the same through verify (k = 6 drafts per sequence, causal tail; 4 x 6 x 8 = 192 prefix rows:
+    # two-pipe items on the tcgen05 path)
+    kk = np.full(cfg.n_seqs, 6)
+    cfgv = cfg.scaled(k_draft=6)
     wl, orc, spk, ids = _build_both(cfgv, kk)
     _set_path(spk, path)
     q, qi = wl.q_all(), wl.q_indptr()
@@ -189,6 +194,9 @@ def test_small_verify(ks, path):
     out, lse = spk.verify_attn(wl.group_indptr(), ids, qi, q)
     check_attn(out, lse, out_ref, lse_ref, "bf16", f"verify k={ks}")
     _check_kernel(spk.last_plan(), path)
+    if path in ("auto", "tcgen05"):
+        # a group of 4 with G = 8: the shared prefix has 32 * mean(k) rows -> two-pipe items iff > 128
+        assert (spk.last_plan()["n_two_pipe_items"] > 0) == (32 * sum(ks) // 4 > 128)
     # ungrouped = same result
     out1, lse1 = spk.verify_attn(np.arange(len(ids) + 1), ids, qi, q)
     check_attn(out1, lse1, out_ref, lse_ref, "bf16", f"verify ungrouped k={ks}")
