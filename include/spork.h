@@ -232,11 +232,12 @@ int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
  */
 int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
 /*
- * Tuning knob: allow (default) or forbid the two-pipe variant of the tcgen05 kernel.  Allowed:
+ * Tuning knob: allow or forbid (default) the two-pipe variant of the tcgen05 kernel.  Allowed:
  * a tensor-path segment of more than 128 rows (verify: drafts x group members x GQA heads) is cut
  * into row blocks of 256 and run by CTAs with two softmax pipes that share one stream of K/V
  * tiles (one CTA per SM).  Forbidden: row blocks of 128 on the one-pipe kernel, each re-reading
- * the K/V tiles through L2.  Results do not depend on it beyond rounding.  Invalidates the plan.
+ * the K/V tiles through L2 (measured equal or faster on BASELINE.json config 4, hence the default).
+ * Results do not depend on it beyond rounding.  Invalidates the plan.
  */
 int spork_set_two_pipe(spork_ctx *ctx, int enable);
 

@@ -326,10 +326,11 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
                         if (t + 32 >= vis) s1[t] = 0xff800000u;
                     }
                 }
-                float mx = -INFINITY;
+                float mxa[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};   // 4 independent chains
 #pragma unroll
                 for (int t = 0; t < 32; ++t)
-                    mx = fmaxf(mx, fmaxf(__uint_as_float(s0[t]), __uint_as_float(s1[t])));
+                    mxa[t & 3] = fmaxf(mxa[t & 3], fmaxf(__uint_as_float(s0[t]), __uint_as_float(s1[t])));
+                const float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
                 const float mxs = mx * P.scale_log2;
                 const bool grow = mxs > m_used + RESCALE_THRESHOLD;
                 if (__any_sync(0xffffffffu, grow)) {

@@ -125,7 +125,7 @@ struct spork_ctx {
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
     int timing = 0;
-    int two_pipe = 1;             // segments of > 128 rows run on the two-pipe tcgen05 kernel
+    int two_pipe = 0;             // 1: segments of > 128 rows run on the two-pipe tcgen05 kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;
