@@ -253,61 +253,60 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
         const uint32_t tO = tbase + w * PIPE_COLS;
         const int st = threadIdx.x - 64;               // 0 .. N_SOFTMAX-1 among the softmax threads
         uint32_t g0 = 0, gt = 0;                       // tiles this pipe has run / tiles of all items so far
+        // Q rows of an item -> smem (K-major, 128-byte swizzle); rows beyond nrows are zero.  Each pipe
+        // stages its own 128 rows.  All 16 loads of a thread are in flight together.  Called for the
+        // NEXT item as soon as this thread has seen the last S of the current item complete (its Q
+        // image is then dead), i.e. before the epilogue: the global-load latency and the next item's
+        // first S MMA hide under the last P V and the write-back of the partials.
+        auto stage_q = [&](const WorkItem &qi) {
+            const int c = st & 15;                     // 16-byte chunk of the row
+            uint4 v[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const int row = w * 128 + ((st & 127) >> 4) + 8 * k;
+                v[k] = make_uint4(0, 0, 0, 0);
+                if (row < qi.nrows) {
+                    const int lr = qi.rb0 + row;
+                    const uint16_t *src =
+                        P.q + ((size_t)(qi.qrow0 + lr / P.G) * P.Hq + qi.kvh * P.G + lr % P.G) * D + c * 8;
+                    v[k] = *reinterpret_cast<const uint4 *>(src);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+                const int rp = ((st & 127) >> 4) + 8 * k;   // row inside the pipe's 32 KiB image
+                const int off = w * Q_BYTES + (c >> 3) * Q_HALF + (rp >> 3) * 1024 + (rp & 7) * 128 +
+                                (((c & 7) ^ (rp & 7)) << 4);
+                *reinterpret_cast<uint4 *>(smem + off) = v[k];
+            }
+            fence_async_smem();
+            asm volatile("bar.sync 1, %0;" ::"n"(C::N_SOFTMAX) : "memory");
+            if (st == 0) mbar_arrive(bar(C::B_QFULL));
+        };
+        if (item_begin < item_end) stage_q(P.items[item_begin]);
         for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = P.items[idx];
+            const bool has_next = idx + 1 < item_end;
             const int n_tok = it.tok1 - it.tok0;
             const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
-            // ---- Q rows -> smem (K-major, 128-byte swizzle); rows beyond nrows are zero ----
-            {
-                // each pipe stages its own 128 rows: its previous Q image is free once ITS last P V of the
-                // previous item has completed, whatever the other pipe is still doing
-                const int c = st & 15;                 // 16-byte chunk of the row
-#pragma unroll 4
-                for (int k = 0; k < 16; ++k) {
-                    const int row = w * 128 + ((st & 127) >> 4) + 8 * k;
-                    uint4 v = make_uint4(0, 0, 0, 0);
-                    if (row < it.nrows) {
-                        const int lr = it.rb0 + row;
-                        const uint16_t *src =
-                            P.q + ((size_t)(it.qrow0 + lr / P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D + c * 8;
-                        v = *reinterpret_cast<const uint4 *>(src);
-                    }
-                    const int rp = row & 127;          // row inside its pipe's 32 KiB image
-                    const int off = (row >> 7) * Q_BYTES + (c >> 3) * Q_HALF + (rp >> 3) * 1024 + (rp & 7) * 128 +
-                                    (((c & 7) ^ (rp & 7)) << 4);
-                    *reinterpret_cast<uint4 *>(smem + off) = v;
-                }
-                fence_async_smem();
-                asm volatile("bar.sync 1, %0;" ::"n"(C::N_SOFTMAX) : "memory");
-                if (st == 0) mbar_arrive(bar(C::B_QFULL));
-            }
-            if (NP > 1 && w * 128 >= it.nrows) {       // this pipe sits the item out (the MMA thread knows)
-                gt += n_tiles;
-                continue;
-            }
+            // 0: this pipe sits the item out (NP = 2, <= 128 rows: the MMA warp knows); 1: none of this warp's
+            // 32 rows exists (few-row item): only keep the barriers moving, whatever S/P/O hold in these
+            // lanes never leaves TMEM; 2: softmax
+            const int mode = (NP > 1 && w * 128 >= it.nrows) ? 0 : (w * 128 + lg * 32 >= it.nrows ? 1 : 2);
             const int lim_r = it.lim0 + (it.rb0 + r) / P.G;
             const int min_lim = it.lim0 + (it.rb0 + w * 128) / P.G;
             float m_used = -INFINITY, l = 0.f, lr = 0.f;   // l: exact row sum (lse); lr: sum of the bf16 weights
 
-            if (w * 128 + lg * 32 >= it.nrows) {
-                // none of this warp's 32 rows exists (few-row item): only keep the barriers moving;
-                // whatever S/P/O hold in these lanes never leaves TMEM
+            if (mode == 1) {
                 for (int i = 0; i < n_tiles; ++i) {
                     const uint32_t g = g0 + i, b = g & 1;
                     mbar_wait(pbar(w, P_SFULL + b), (g >> 1) & 1);
                     if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
                     __syncwarp();
                 }
-                const uint32_t gl = g0 + n_tiles - 1;
-                mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
-                if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
-                __syncwarp();
-                g0 += n_tiles;
-                gt += n_tiles;
-                continue;
             }
 
-            for (int i = 0; i < n_tiles; ++i) {
+            for (int i = 0; mode == 2 && i < n_tiles; ++i) {
                 const uint32_t g = g0 + i, b = g & 1;
                 const uint32_t tS = tO + 128 + 64 * b + lane_addr;
                 mbar_wait(pbar(w, P_SFULL + b), (g >> 1) & 1);
@@ -400,8 +399,16 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
                 if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
             }
 
+            if (has_next) stage_q(P.items[idx + 1]);
+
+            if (mode == 1) {
+                const uint32_t gl = g0 + n_tiles - 1;
+                mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
+                __syncwarp();
+            }
             // ---- epilogue: O / l -> partial rows ------------------------------------------------
-            {
+            if (mode == 2) {
                 const uint32_t gl = g0 + n_tiles - 1;
                 mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
                 tc_fence_after();
@@ -426,7 +433,7 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
                 __syncwarp();
                 if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
             }
-            g0 += n_tiles;
+            if (mode != 0) g0 += n_tiles;
             gt += n_tiles;
         }
     }
