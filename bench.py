@@ -211,7 +211,7 @@ def run_ours(args, cfg, name, wl):
     if args.min_rows is not None:
         spk.set_tensor_path_min_rows(args.min_rows)
     if args.two_pipe is not None:
-        spk.set_two_pipe(bool(args.two_pipe))
+        spk.set_two_pipe(args.two_pipe)
     st = spk.stream
     gi = wl.group_indptr()
     qi = wl.q_indptr()
@@ -417,7 +417,7 @@ def main():
     ap.add_argument("--ref-groups", type=int, default=0,
                     help="fork groups in the oracle's bounded sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--two-pipe", type=int, default=None, choices=[0, 1],
+    ap.add_argument("--two-pipe", type=int, default=None, choices=[0, 1, 2],
                     help="planner knob: > 128-row segments on the two-pipe tcgen05 kernel")
     ap.add_argument("--min-rows", type=int, default=None,
                     help="planner knob: rows per KV head from which a segment runs on the tcgen05 kernel")

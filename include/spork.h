@@ -232,14 +232,18 @@ int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
  */
 int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
 /*
- * Tuning knob: allow or forbid (default) the two-pipe variant of the tcgen05 kernel.  Allowed:
- * a tensor-path segment of more than 128 rows (verify: drafts x group members x GQA heads) is cut
- * into row blocks of 256 and run by CTAs with two softmax pipes that share one stream of K/V
- * tiles (one CTA per SM).  Forbidden: row blocks of 128 on the one-pipe kernel, each re-reading
- * the K/V tiles through L2 (measured equal or faster on BASELINE.json config 4, hence the default).
- * Results do not depend on it beyond rounding.  Invalidates the plan.
+ * Tuning knob: which tcgen05 kernel variant runs a tensor-path segment of more than 128 rows
+ * (verify: drafts x group members x GQA heads).  mode 0 (default): the one-pipe kernel in row
+ * blocks of 128, each block re-reading the K/V tiles through L2.  mode 1: row blocks of 256 on
+ * the two-pipe variant (one CTA per SM, two softmax pipes share one stream of K/V tiles).
+ * mode 2: row blocks of 128 on the split-row variant (each row's 64 scores of a tile shared by
+ * two threads, 8 softmax warps per CTA).  Measured on BASELINE.json config 4: mode 0 is equal or
+ * faster (k = 8: 342 / 410 / 430 us, k = 16: 671 / 730 / 712 us for modes 0 / 1 / 2), hence the
+ * default; the variants stay for the next round's tuning and are covered by the parity tests.
+ * Results do not depend on the mode beyond rounding.  Other values are read as 0.  Invalidates
+ * the cached plan.
  */
-int spork_set_two_pipe(spork_ctx *ctx, int enable);
+int spork_set_two_pipe(spork_ctx *ctx, int mode);
 
 const char *spork_strerror(int code);
 

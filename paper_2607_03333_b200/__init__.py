@@ -319,7 +319,7 @@ class Spork:
 
     def set_two_pipe(self, enable: bool):
         """Planner knob: run > 128-row segments on the two-pipe tcgen05 kernel (default on)."""
-        self._chk(self.lib.spork_set_two_pipe(self._h, int(bool(enable))))
+        self._chk(self.lib.spork_set_two_pipe(self._h, int(enable)))
 
     def last_kernel_ms(self):
         """(attention kernel ms, merge kernel ms) of the last attention call (synchronises)."""

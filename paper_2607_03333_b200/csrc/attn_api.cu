@@ -125,7 +125,7 @@ extern "C" int spork_set_tensor_path_min_rows(spork_ctx *c, int min_rows) {
 
 extern "C" int spork_set_two_pipe(spork_ctx *c, int enable) {
     if (!c) return SPORK_ERR_INVALID;
-    c->two_pipe = enable ? 1 : 0;
+    c->two_pipe = enable < 0 || enable > 2 ? 0 : enable;
     c->plan.valid = false;
     return SPORK_OK;
 }

@@ -42,10 +42,14 @@ constexpr float RESCALE_THRESHOLD = 8.f;              // log2 units
 //   NP = 1: items of <= 128 rows, 2 CTAs per SM, 5-slot ring each
 //   NP = 2: items of <= 256 rows (verify with many drafts), 1 CTA per SM, 10-slot ring; every
 //           K/V tile is fetched once for both row blocks
-template <int NP>
+//   SP = 2 (NP = 1 only): every row's 64 scores of a tile are split over TWO threads (8 softmax warps,
+//           4 per SM sub-partition instead of 2) for items whose time is the softmax's, not HBM's:
+//           4-slot ring, the row max and the row sums are exchanged through shared memory
+template <int NP, int SP>
 struct Cfg {
-    static constexpr int NSLOT = NP == 1 ? 5 : 10;
-    static constexpr int N_SOFTMAX = NP * 128;
+    static_assert(SP == 1 || NP == 1, "split rows only with one pipe");
+    static constexpr int NSLOT = NP == 2 ? 10 : (SP == 2 ? 4 : 5);
+    static constexpr int N_SOFTMAX = NP * 128 * SP;
     static constexpr int N_THREADS = 64 + N_SOFTMAX;
     static constexpr int CTAS_PER_SM = NP == 1 ? 2 : 1;
     static constexpr int TMEM_COLS = NP * PIPE_COLS;
@@ -57,7 +61,8 @@ struct Cfg {
     static constexpr int B_PIPE = 2 * NSLOT;          // per pipe: 7 barriers, see P_*
     static constexpr int B_QFULL = B_PIPE + 7 * NP;   // Q staged
     static constexpr int B_COUNT = B_QFULL + 1;
-    static constexpr int SMEM_BYTES = BAR_OFF + 8 * B_COUNT + 16;
+    static constexpr int XCH_OFF = BAR_OFF + 8 * B_COUNT + 16;     // float [2][2][128] (SP = 2)
+    static constexpr int SMEM_BYTES = XCH_OFF + (SP == 2 ? 2048 : 0);
 };
 enum : int {
     P_SFULL = 0,    // [2] S(b) complete
@@ -77,9 +82,10 @@ struct UParams {
     float *ws_o, *ws_lse;
 };
 
-template <int NP>
-__global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn_umma_kernel(const UParams P) {
-    using C = Cfg<NP>;
+template <int NP, int SP>
+__global__ void __launch_bounds__(Cfg<NP, SP>::N_THREADS, Cfg<NP, SP>::CTAS_PER_SM)
+attn_umma_kernel(const UParams P) {
+    using C = Cfg<NP, SP>;
     constexpr int NSLOT = C::NSLOT;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -99,10 +105,10 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
         for (int w = 0; w < NP; ++w) {
             for (int b = 0; b < 2; ++b) {
                 mbar_init(pbar(w, P_SFULL + b), 1);
-                mbar_init(pbar(w, P_PFULL + b), 4);
+                mbar_init(pbar(w, P_PFULL + b), 4 * SP);
                 mbar_init(pbar(w, P_PVDONE + b), 1);
             }
-            mbar_init(pbar(w, P_OFREE), 4);
+            mbar_init(pbar(w, P_OFREE), 4 * SP);
         }
         mbar_init(bar(C::B_QFULL), 1);
         mbar_fence_init();
@@ -247,6 +253,7 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
     } else {
         // ================================ softmax warps ================================
         const int w = NP > 1 ? (warp - 2) >> 2 : 0;    // pipe: rows [128 w, 128 w + 128) of the item
+        const int h = SP > 1 ? (warp - 2) >> 2 : 0;    // SP = 2: which 32 of a tile's 64 scores this thread owns
         const int lg = warp & 3;                       // TMEM lane group this warp may access
         const int r = w * 128 + lg * 32 + lane;        // query row of the item owned by this thread
         const uint32_t lane_addr = (uint32_t)(lg * 32) << 16;
@@ -260,10 +267,11 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
         // first S MMA hide under the last P V and the write-back of the partials.
         auto stage_q = [&](const WorkItem &qi) {
             const int c = st & 15;                     // 16-byte chunk of the row
-            uint4 v[16];
+            constexpr int QT = 128 * SP, NK = 16 / SP;  // threads staging one pipe's image, rows per thread
+            uint4 v[NK];
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                const int row = w * 128 + ((st & 127) >> 4) + 8 * k;
+            for (int k = 0; k < NK; ++k) {
+                const int row = w * 128 + ((st & (QT - 1)) >> 4) + (QT / 16) * k;
                 v[k] = make_uint4(0, 0, 0, 0);
                 if (row < qi.nrows) {
                     const int lr = qi.rb0 + row;
@@ -273,8 +281,8 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
                 }
             }
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
-                const int rp = ((st & 127) >> 4) + 8 * k;   // row inside the pipe's 32 KiB image
+            for (int k = 0; k < NK; ++k) {
+                const int rp = ((st & (QT - 1)) >> 4) + (QT / 16) * k;   // row inside the pipe's 32 KiB image
                 const int off = w * Q_BYTES + (c >> 3) * Q_HALF + (rp >> 3) * 1024 + (rp & 7) * 128 +
                                 (((c & 7) ^ (rp & 7)) << 4);
                 *reinterpret_cast<uint4 *>(smem + off) = v[k];
@@ -304,6 +312,142 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
                     if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
                     __syncwarp();
                 }
+            }
+
+            if constexpr (SP == 2) {
+                // ---- split rows: this thread owns scores [32 h, 32 h + 32) of its row in every tile ----
+                float *xch = reinterpret_cast<float *>(smem + C::XCH_OFF);      // [2][2][128]
+                auto pair_sync = [&]() {                 // the two warps that share TMEM lane group lg
+                    asm volatile("bar.sync %0, 64;" ::"r"(2 + lg) : "memory");
+                };
+                const int rr = lg * 32 + lane;
+                for (int i = 0; mode == 2 && i < n_tiles; ++i) {
+                    const uint32_t g = g0 + i, b = g & 1;
+                    const uint32_t tS = tO + 128 + 64 * b + lane_addr;
+                    mbar_wait(pbar(w, P_SFULL + b), (g >> 1) & 1);
+                    tc_fence_after();
+                    uint32_t sc[32];
+                    tmem_ld32(tS + 32 * h, sc);
+                    tmem_wait_ld();
+                    const int tile_t0 = it.tok0 + i * TILE_TOKENS;
+                    const int nv = min(TILE_TOKENS, it.tok1 - tile_t0);
+                    if (nv < TILE_TOKENS || tile_t0 + TILE_TOKENS - 1 > min_lim) {
+                        const int vis = min(nv, lim_r - tile_t0 + 1) - 32 * h;
+#pragma unroll
+                        for (int t = 0; t < 32; ++t)
+                            if (t >= vis) sc[t] = 0xff800000u;           // -inf
+                    }
+                    float mxa[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+                    for (int t = 0; t < 32; ++t) mxa[t & 3] = fmaxf(mxa[t & 3], __uint_as_float(sc[t]));
+                    float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
+                    // row max over both halves (double buffered by tile parity: a thread is at most one
+                    // pair barrier ahead of its partner)
+                    xch[((g & 1) * 2 + h) * 128 + rr] = mx;
+                    pair_sync();
+                    mx = fmaxf(mx, xch[((g & 1) * 2 + (h ^ 1)) * 128 + rr]);
+                    const float mxs = mx * P.scale_log2;
+                    const bool grow = mxs > m_used + RESCALE_THRESHOLD;
+                    if (__any_sync(0xffffffffu, grow)) {          // same rows, same values: both halves agree
+                        const float m_new = grow ? mxs : m_used;
+                        const float alpha = grow ? (m_used == -INFINITY ? 0.f : ex2(m_used - m_new)) : 1.f;
+                        l *= alpha;
+                        lr *= alpha;
+                        if (i > 0) {
+                            mbar_wait(pbar(w, P_PVDONE + ((g - 1) & 1)), ((g - 1) >> 1) & 1);
+                            tc_fence_after();
+#pragma unroll 1
+                            for (int cb = 2 * h; cb < 2 * h + 2; ++cb) {     // this half's 64 columns of O
+                                uint32_t o[32];
+                                tmem_ld32(tO + lane_addr + cb * 32, o);
+                                tmem_wait_ld();
+#pragma unroll
+                                for (int t = 0; t < 32; ++t) o[t] = __float_as_uint(__uint_as_float(o[t]) * alpha);
+                                tmem_st32(tO + lane_addr + cb * 32, o);
+                            }
+                            tmem_wait_st();
+                        }
+                        m_used = m_new;
+                    }
+                    const float mu = m_used == -INFINITY ? 0.f : m_used;
+                    uint32_t p[16];
+                    float sum0 = 0.f, sum1 = 0.f, rs0 = 0.f, rs1 = 0.f;
+#pragma unroll
+                    for (int t = 0; t < 8; ++t) {
+                        const float a0 = ex2(fmaf(__uint_as_float(sc[4 * t]), P.scale_log2, -mu));
+                        const float a1 = ex2(fmaf(__uint_as_float(sc[4 * t + 1]), P.scale_log2, -mu));
+                        const float c0 = ex2(fmaf(__uint_as_float(sc[4 * t + 2]), P.scale_log2, -mu));
+                        const float c1 = ex2(fmaf(__uint_as_float(sc[4 * t + 3]), P.scale_log2, -mu));
+                        p[2 * t] = pack_bf16(a0, a1);
+                        p[2 * t + 1] = pack_bf16(c0, c1);
+                        sum0 += a0 + a1;
+                        sum1 += c0 + c1;
+                        rs0 += __uint_as_float(p[2 * t] << 16) + __uint_as_float(p[2 * t] & 0xffff0000u);
+                        rs1 += __uint_as_float(p[2 * t + 1] << 16) + __uint_as_float(p[2 * t + 1] & 0xffff0000u);
+                    }
+                    l += sum0 + sum1;
+                    lr += rs0 + rs1;
+                    // P columns [16 h, 16 h + 16) lie over S columns both halves have already read
+                    tmem_st16(tS + 16 * h, p);
+                    tmem_wait_st();
+                    if ((nv & (PS - 1)) && lg == 0 && h == 0) {
+                        const uint32_t ldv = 2 * (gt + i) + 1, slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
+                        mbar_wait(bar(C::B_FULL + slot), ph);
+                        const int nvp = (nv + PS - 1) / PS;
+                        uint8_t *vpage = smem + C::RING_OFF + slot * SLOT_BYTES + (nvp - 1) * HEAD_BLOCK;
+                        const int r_first = nv & (PS - 1);
+                        for (int e = lane; e < (PS - r_first) * 16; e += 32) {
+                            const int r2 = r_first + (e >> 4), cc = e & 15;
+                            *reinterpret_cast<uint4 *>(vpage + swz_chunk_off(2, r2, cc)) = make_uint4(0, 0, 0, 0);
+                        }
+                        fence_async_smem();
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
+                }
+                if (has_next) stage_q(P.items[idx + 1]);
+                if (mode == 1) {
+                    const uint32_t gl = g0 + n_tiles - 1;
+                    mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                    if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
+                    __syncwarp();
+                }
+                if (mode == 2) {
+                    const uint32_t gl = g0 + n_tiles - 1;
+                    mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
+                    tc_fence_after();
+                    pair_sync();                                   // the partner has read the last row max
+                    xch[(0 * 2 + h) * 128 + rr] = l;
+                    xch[(1 * 2 + h) * 128 + rr] = lr;
+                    pair_sync();
+                    l += xch[(0 * 2 + (h ^ 1)) * 128 + rr];
+                    lr += xch[(1 * 2 + (h ^ 1)) * 128 + rr];
+                    pair_sync();                                   // ... before the next item's first tile
+                    const float inv = lr > 0.f ? 1.f / lr : 0.f;
+                    float *dst = P.ws_o + (size_t)(it.part_base + r) * D;
+#pragma unroll 1
+                    for (int cb = 2 * h; cb < 2 * h + 2; ++cb) {
+                        uint32_t o[32];
+                        tmem_ld32(tO + lane_addr + cb * 32, o);
+                        tmem_wait_ld();
+                        if (r < it.nrows) {
+#pragma unroll
+                            for (int t = 0; t < 8; ++t)
+                                *reinterpret_cast<float4 *>(dst + cb * 32 + 4 * t) =
+                                    make_float4(__uint_as_float(o[4 * t]) * inv, __uint_as_float(o[4 * t + 1]) * inv,
+                                                __uint_as_float(o[4 * t + 2]) * inv, __uint_as_float(o[4 * t + 3]) * inv);
+                        }
+                    }
+                    if (r < it.nrows && h == 0)
+                        P.ws_lse[it.part_base + r] = l > 0.f ? (m_used + log2f(l)) * LN2 : -INFINITY;
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(pbar(w, P_OFREE));
+                }
+                if (mode != 0) g0 += n_tiles;
+                gt += n_tiles;
+                continue;
             }
 
             for (int i = 0; mode == 2 && i < n_tiles; ++i) {
@@ -455,35 +599,36 @@ __global__ void __launch_bounds__(Cfg<NP>::N_THREADS, Cfg<NP>::CTAS_PER_SM) attn
 
 namespace spork {
 
-int attn_umma_grid(spork_ctx *c, int np) {
-    return c->num_sms * (np == 1 ? Cfg<1>::CTAS_PER_SM : Cfg<2>::CTAS_PER_SM);
+// variant 0: one pipe (the default kernel), 1: two pipes, 2: one pipe with split rows
+int attn_umma_grid(spork_ctx *c, int variant) {
+    return c->num_sms * (variant == 1 ? Cfg<2, 1>::CTAS_PER_SM : Cfg<1, 1>::CTAS_PER_SM);
 }
 
-template <int NP>
+template <int NP, int SP>
 static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic, cudaStream_t st) {
     static bool attr_set = false;
     if (!attr_set) {
-        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        Cfg<NP>::SMEM_BYTES));
+        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg<NP, SP>::SMEM_BYTES));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(Cfg<NP>::N_THREADS);
-    cfg.dynamicSmemBytes = Cfg<NP>::SMEM_BYTES;
+    cfg.blockDim = dim3(Cfg<NP, SP>::N_THREADS);
+    cfg.dynamicSmemBytes = Cfg<NP, SP>::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = programmatic ? 1 : 0;   // may start while the previous attention kernel drains
-    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP>, p));
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP, SP>, p));
     c->last_launches++;
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;
 }
 
-// np = 2: the <= 256-row items (launched first), np = 1: the <= 128-row items
+// np = 2: the many-row items' list (launched first; two-pipe or split-row kernel), np = 1: the others
 int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st) {
     const Plan &P = c->plan;
     const int n = np == 2 ? P.n_items_umma2 : P.n_items_umma;
@@ -503,8 +648,9 @@ int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cud
     p.scale_log2 = c->cfg.scale * LOG2E;
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
-    return np == 2 ? launch_np<2>(c, p, P.grid_umma2, programmatic, st)
-                   : launch_np<1>(c, p, P.grid_umma, programmatic, st);
+    if (np == 1) return launch_np<1, 1>(c, p, P.grid_umma, programmatic, st);
+    return P.variant2 == 2 ? launch_np<1, 2>(c, p, P.grid_umma2, programmatic, st)
+                           : launch_np<2, 1>(c, p, P.grid_umma2, programmatic, st);
 }
 
 }  // namespace spork

@@ -79,6 +79,7 @@ struct Plan {
     int n_items = 0, n_qrows = 0, grid = 0;
     int n_items_umma = 0, grid_umma = 0;
     int n_items_umma2 = 0, grid_umma2 = 0;
+    int variant2 = 1;           // kernel of the second tcgen05 list: 1 two pipes, 2 split rows
     spork_plan_info info{};
 };
 
@@ -125,7 +126,7 @@ struct spork_ctx {
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
     int timing = 0;
-    int two_pipe = 0;             // 1: segments of > 128 rows run on the two-pipe tcgen05 kernel
+    int two_pipe = 0;             // segments of > 128 rows: 0 default kernel, 1 two-pipe, 2 split-row kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;
@@ -161,7 +162,7 @@ int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st);
 int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st);
 int attn_mma_grid(spork_ctx *c);
 int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st);
-int attn_umma_grid(spork_ctx *c, int np);
+int attn_umma_grid(spork_ctx *c, int variant);
 int launch_attn_mma(spork_ctx *c, const void *q, bool programmatic, cudaStream_t st);
 
 // Swizzled (page, kv head) block, bf16 with D % 64 == 0: the block is a run of 1 KiB

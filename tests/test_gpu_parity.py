@@ -93,20 +93,22 @@ SMALL_DECODE = [
 
 
 # planner knob: which segments run on the tcgen05 kernel (None = default threshold)
-PATHS = {"auto": None, "tcgen05": 1, "tcgen05-two-pipe": 1, "mma.sync": 1 << 20}
+PATHS = {"auto": None, "tcgen05": 1, "tcgen05-two-pipe": 1, "tcgen05-split-row": 1, "mma.sync": 1 << 20}
 
 
 def _set_path(spk, path):
     if PATHS[path] is not None:
         spk.set_tensor_path_min_rows(PATHS[path])
     if path == "tcgen05-two-pipe":
-        spk.set_two_pipe(True)
+        spk.set_two_pipe(1)
+    if path == "tcgen05-split-row":
+        spk.set_two_pipe(2)
 
 
 def _check_kernel(info, path):
     if path.startswith("tcgen05"):
         assert info["kernel"] == 2 and info["n_umma_items"] == info["n_items"]
-        if path != "tcgen05-two-pipe":
+        if path == "tcgen05":
             assert info["n_two_pipe_items"] == 0
     elif path == "mma.sync":
         assert info["kernel"] == 1 and info["n_umma_items"] == 0
@@ -139,7 +141,7 @@ def test_small_bf16_decode(cfg, path):
     assert np.array_equal(out1.cpu().numpy(), out_b.cpu().numpy())
 
 
-@pytest.mark.parametrize("path", ["tcgen05", "tcgen05-two-pipe", "mma.sync"])
+@pytest.mark.parametrize("path", ["tcgen05", "tcgen05-two-pipe", "tcgen05-split-row", "mma.sync"])
 @pytest.mark.parametrize("frac,scale", [(0.01, 8.0), (0.05, 16.0), (0.3, 4.0)])
 def test_outlier_keys_running_max_jumps(frac, scale, path):
     """Attention-sink outliers (BASELINE.json config 3): the running row max jumps by far more than
@@ -194,7 +196,7 @@ def test_small_verify(ks, path):
     out, lse = spk.verify_attn(wl.group_indptr(), ids, qi, q)
     check_attn(out, lse, out_ref, lse_ref, "bf16", f"verify k={ks}")
     _check_kernel(spk.last_plan(), path)
-    if path == "tcgen05-two-pipe":
+    if path in ("tcgen05-two-pipe", "tcgen05-split-row"):
         # a group of 4 with G = 8: the shared prefix has 32 * mean(k) rows -> two-pipe items iff > 128
         assert (spk.last_plan()["n_two_pipe_items"] > 0) == (32 * sum(ks) // 4 > 128)
     # ungrouped = same result
