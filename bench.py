@@ -210,6 +210,8 @@ def run_ours(args, cfg, name, wl):
     t_build = time.perf_counter() - t_build
     if args.min_rows is not None:
         spk.set_tensor_path_min_rows(args.min_rows)
+    if args.stream_k is not None:
+        spk.set_stream_k(bool(args.stream_k))
     if args.two_pipe is not None:
         spk.set_two_pipe(args.two_pipe)
     st = spk.stream
@@ -417,6 +419,7 @@ def main():
     ap.add_argument("--ref-groups", type=int, default=0,
                     help="fork groups in the oracle's bounded sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stream-k", type=int, default=None, choices=[0, 1], help="planner knob: stream-K schedule")
     ap.add_argument("--two-pipe", type=int, default=None, choices=[0, 1, 2],
                     help="planner knob: > 128-row segments on the two-pipe tcgen05 kernel")
     ap.add_argument("--min-rows", type=int, default=None,

@@ -205,8 +205,8 @@ typedef struct spork_plan_info {
     int64_t partial_rows;   /* rows of split-KV workspace written                   */
     int32_t launches;       /* kernels launched by the last attention call          */
     int32_t n_umma_items;   /* of n_items, those run by the tcgen05 kernels         */
-    int32_t n_two_pipe_items; /* of those, items of <= 256 rows on the two-pipe variant */
-    int32_t reserved;
+    int32_t n_two_pipe_items; /* of those, items on the second tcgen05 list (knob)   */
+    int32_t stream_k;       /* 1: equal-work contiguous schedule    */
 } spork_plan_info;
 int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
 /* kernels launched by the last state call (append / fork / release / truncate) */
@@ -244,6 +244,15 @@ int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
  * the cached plan.
  */
 int spork_set_two_pipe(spork_ctx *ctx, int mode);
+/*
+ * Tuning knob: allow (default) or forbid the stream-K schedule.  Allowed: when every segment of
+ * a call is a single row block of the tcgen05 kernel (every decode call on a bf16, D = 128
+ * context; verify with few drafts), the (segment, kv head) streams are laid end to end and cut
+ * into one contiguous, equal-cost run per persistent CTA.  Forbidden, or for other calls: equal
+ * chunks per segment, longest-processing-time-first onto the CTAs.  Results do not depend on it
+ * beyond rounding.  Invalidates the cached plan.
+ */
+int spork_set_stream_k(spork_ctx *ctx, int enable);
 
 const char *spork_strerror(int code);
 

@@ -32,7 +32,7 @@ ABI_SYMBOLS = [
     "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
-    "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_strerror",
+    "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
 ]
 
 
@@ -47,7 +47,7 @@ class PlanInfo(C.Structure):
                 ("grid", C.c_int32), ("kernel", C.c_int32), ("plan_cached", C.c_int32),
                 ("unique_tokens", C.c_int64), ("naive_tokens", C.c_int64),
                 ("partial_rows", C.c_int64), ("launches", C.c_int32), ("n_umma_items", C.c_int32),
-                ("n_two_pipe_items", C.c_int32), ("reserved", C.c_int32)]
+                ("n_two_pipe_items", C.c_int32), ("stream_k", C.c_int32)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
@@ -93,6 +93,7 @@ def load(build_if_missing: bool = True):
         "spork_set_timing": ([P, I], I),
         "spork_set_tensor_path_min_rows": ([P, I], I),
         "spork_set_two_pipe": ([P, I], I),
+        "spork_set_stream_k": ([P, I], I),
         "spork_last_kernel_ms": ([P, P, P], I),
         "spork_strerror": ([I], C.c_char_p),
     }
@@ -320,6 +321,10 @@ class Spork:
     def set_two_pipe(self, enable: bool):
         """Planner knob: run > 128-row segments on the two-pipe tcgen05 kernel (default on)."""
         self._chk(self.lib.spork_set_two_pipe(self._h, int(enable)))
+
+    def set_stream_k(self, enable: bool):
+        """Planner knob: equal-work contiguous schedule for single-row-block calls (default on)."""
+        self._chk(self.lib.spork_set_stream_k(self._h, int(bool(enable))))
 
     def last_kernel_ms(self):
         """(attention kernel ms, merge kernel ms) of the last attention call (synchronises)."""

@@ -129,3 +129,10 @@ extern "C" int spork_set_two_pipe(spork_ctx *c, int enable) {
     c->plan.valid = false;
     return SPORK_OK;
 }
+
+extern "C" int spork_set_stream_k(spork_ctx *c, int enable) {
+    if (!c) return SPORK_ERR_INVALID;
+    c->stream_k = enable ? 1 : 0;
+    c->plan.valid = false;
+    return SPORK_OK;
+}

@@ -146,15 +146,17 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
 // Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
 // every load of a batch in flight before the first use (the kernel is pure L2 latency).
 template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
-__global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__ qd, int n_qrows, int Hq,
+__global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__ qd,
+                                                    const StreamDesc *__restrict__ streams, int n_qrows, int Hq,
                                                     int G, int D, const float *ws_o, const float *ws_lse,
                                                     float *__restrict__ out, float *__restrict__ lse) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= n_qrows * Hq) return;
     const int qrow = w / Hq, h = w % Hq;
     const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
+    const RowStreams rs = load_row_streams(streams, d, h / G);
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    merge_row<NI>(d, h / G, h % G, G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
+    merge_row<NI>(rs, d, h % G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
 }
 
 }  // namespace
@@ -203,7 +205,7 @@ int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     SPORK_CUDA(cudaLaunchKernelEx(&cfg, c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>,
-                                  (const QRowDesc *)P.qdesc.p, P.n_qrows,
+                                  (const QRowDesc *)P.qdesc.p, (const StreamDesc *)P.streams.p, P.n_qrows,
                                   (int)c->cfg.num_q_heads, c->G, (int)c->cfg.head_dim,
                                   (const float *)c->ws_o.p, (const float *)c->ws_lse.p, out, lse));
     c->last_launches++;

@@ -447,8 +447,7 @@ attn_umma_kernel(const UParams P) {
                 }
                 if (mode != 0) g0 += n_tiles;
                 gt += n_tiles;
-                continue;
-            }
+            } else {
 
             for (int i = 0; mode == 2 && i < n_tiles; ++i) {
                 const uint32_t g = g0 + i, b = g & 1;
@@ -579,6 +578,7 @@ attn_umma_kernel(const UParams P) {
             }
             if (mode != 0) g0 += n_tiles;
             gt += n_tiles;
+            }   // SP == 1
         }
     }
 

@@ -19,16 +19,29 @@ __device__ __forceinline__ float merge_warp_max(float v) {
 
 // Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
 // every load of a batch in flight before the first use (pure L2 latency otherwise).
+// The two streams a row draws its partials from (none: nsplit = 0).
+struct RowStreams {
+    StreamDesc pre, suf;
+};
+__device__ __forceinline__ RowStreams load_row_streams(const StreamDesc *__restrict__ streams, const QRowDesc &d,
+                                                       int kvh) {
+    RowStreams r{{0, 0, 0, 0}, {0, 0, 0, 0}};
+    if (d.pre_stream >= 0) r.pre = streams[d.pre_stream + kvh];
+    if (d.suf_stream >= 0) r.suf = streams[d.suf_stream + kvh];
+    return r;
+}
+
 template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
-__device__ __forceinline__ void merge_row(const QRowDesc &d, int kvh, int j, int G, int D,
+__device__ __forceinline__ void merge_row(const RowStreams &rs, const QRowDesc &d, int j, int D,
                                           const float *ws_o, const float *ws_lse, float *out_row,
                                           float *lse_out, int lane) {
-    const int pre0 = d.pre_base + kvh * d.pre_nq * G + d.pre_qi * G + j;
-    const int suf0 = d.suf_base + kvh * d.suf_nq * G + d.suf_qi * G + j;
-    const int n = d.pre_nsplit + d.suf_nsplit;
+    const StreamDesc &pre = rs.pre, &suf = rs.suf;
+    const int pre0 = pre.part_base + d.pre_off + j;
+    const int suf0 = suf.part_base + d.suf_off + j;
+    const int n = pre.nsplit + suf.nsplit;
     auto part = [&](int s) -> size_t {
-        return s < d.pre_nsplit ? (size_t)pre0 + (size_t)s * d.pre_stride
-                                : (size_t)suf0 + (size_t)(s - d.pre_nsplit) * d.suf_stride;
+        return s < pre.nsplit ? (size_t)pre0 + (size_t)s * pre.stride
+                              : (size_t)suf0 + (size_t)(s - pre.nsplit) * suf.stride;
     };
     const float lse_mine = lane < n ? __ldcg(ws_lse + part(lane)) : -INFINITY;   // split `lane`
     float M = lse_mine;

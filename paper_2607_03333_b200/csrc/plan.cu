@@ -210,13 +210,10 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             unique_tokens += L - S;
             for (int j = 0; j < k; ++j) {
                 QRowDesc &d = qd[q0 + j];
-                d = QRowDesc{};
-                d.pre_base = pre_seg;  // segment index for now; resolved below
-                d.pre_nq = gnq;
-                d.pre_qi = q0 + j - gq0;
-                d.suf_base = suf_seg;
-                d.suf_nq = k;
-                d.suf_qi = j;
+                d.pre_stream = pre_seg;  // segment index for now; stream = segment * Hkv (+ kv head)
+                d.pre_off = (q0 + j - gq0) * G;
+                d.suf_stream = suf_seg;
+                d.suf_off = j * G;
             }
         }
     }
@@ -312,69 +309,132 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         if (!split(chunk_tiles, &part_rows, &n_items)) return SPORK_ERR_INVALID;
     }
     for (QRowDesc &d : qd) {
-        if (d.pre_base >= 0) {
-            const Segment &s = segs[d.pre_base];
-            d.pre_base = s.part_base;
-            d.pre_nsplit = s.nsplit;
-            d.pre_stride = s.nq * Hq;
-        } else {
-            d.pre_base = 0;
-            d.pre_nsplit = 0;
-        }
-        if (d.suf_base >= 0) {
-            const Segment &s = segs[d.suf_base];
-            d.suf_base = s.part_base;
-            d.suf_nsplit = s.nsplit;
-            d.suf_stride = s.nq * Hq;
-        } else {
-            d.suf_base = 0;
-            d.suf_nsplit = 0;
-        }
+        if (d.pre_stream >= 0) d.pre_stream *= Hkv;
+        if (d.suf_stream >= 0) d.suf_stream *= Hkv;
     }
+    std::vector<StreamDesc> streams(segs.size() * (size_t)Hkv);   // stream of (segment s, kv head h) = s * Hkv + h
 
-    // ---- items of the two kernels, each longest first and statically scheduled -----------------
     std::vector<WorkItem> items, items_umma, items_umma2;
-    items.reserve(n_items);
+    std::vector<int32_t> cta_ptr, cta_ptr_umma, cta_ptr_umma2;
     int n_prefix_items = 0;
-    for (const Segment &s : segs) {
-        const int rows = s.nq * G;
-        std::vector<WorkItem> &dst = s.kind == 2 ? items_umma2 : (s.kind == 1 ? items_umma : items);
-        for (int sp = 0; sp < s.nsplit; ++sp) {
-            int t0 = s.tok0 + sp * s.chunk_tiles * TILE_TOKENS;
-            int t1 = std::min(s.tok1, t0 + s.chunk_tiles * TILE_TOKENS);
-            for (int h = 0; h < Hkv; ++h)
-                for (int rb = 0; rb < rows; rb += s.row_block) {
-                    WorkItem it{};
-                    it.table_seq = s.table_seq;
-                    it.tok0 = t0;
-                    it.tok1 = t1;
-                    it.kvh = h;
-                    it.qrow0 = s.qrow0;
-                    it.rb0 = rb;
-                    it.nrows = std::min(s.row_block, rows - rb);
-                    it.lim0 = s.lim0;
-                    it.part_base = s.part_base + sp * s.nq * Hq + h * rows + rb;
-                    dst.push_back(it);
-                    n_prefix_items += s.prefix;
+    auto make_item = [&](const Segment &s, int h, int rb, int t0, int t1, int part_base) {
+        WorkItem it{};
+        it.table_seq = s.table_seq;
+        it.tok0 = t0;
+        it.tok1 = t1;
+        it.kvh = h;
+        it.qrow0 = s.qrow0;
+        it.rb0 = rb;
+        it.nrows = std::min(s.row_block, s.nq * G - rb);
+        it.lim0 = s.lim0;
+        it.part_base = part_base;
+        n_prefix_items += s.prefix;
+        return it;
+    };
+
+    // ---- stream-K schedule: when every segment is ONE row block of the one-pipe tcgen05 kernel (all
+    // decode plans, verify with few drafts), the segments are laid end to end, longest first, and cut
+    // into contiguous runs of equal cost (tiles + a fixed cost per piece), one run per gang of Hkv CTAs:
+    // every CTA streams the same number of bytes and a segment is split only where a gang boundary
+    // falls (fewest partials).
+    bool stream_k = mma && c->stream_k && !segs.empty();
+    for (const Segment &s : segs) stream_k = stream_k && s.kind == 1 && s.nq * G <= s.row_block;
+    if (stream_k) {
+        // CTAs work in gangs of Hkv: a gang walks the same token run, CTA h of the gang on kv head h, so
+        // the Hkv blocks of a page (contiguous in the pool) are fetched at the same time
+        struct Str { int seg, tiles; };
+        std::vector<Str> order;
+        order.reserve(segs.size());
+        int64_t tiles_total = 0;
+        for (size_t si = 0; si < segs.size(); ++si) {
+            const int tiles = ceil_div(segs[si].tok1 - segs[si].tok0, TILE_TOKENS);
+            order.push_back({(int)si, tiles});
+            tiles_total += tiles;
+        }
+        std::stable_sort(order.begin(), order.end(), [](const Str &a, const Str &b) { return a.tiles > b.tiles; });
+        const int n_gangs = (int)std::min<int64_t>(std::max(1, grid_cap_umma / Hkv),
+                                                  std::max<int64_t>(1, tiles_total / MIN_CHUNK_TILES));
+        const int G_ = n_gangs * Hkv;
+        const double c0 = ITEM_FIXED_COST_UMMA;
+        const double budget = ((double)tiles_total + c0 * ((double)order.size() + n_gangs)) / n_gangs;
+        std::vector<std::vector<WorkItem>> per_cta(G_);
+        int gang = 0;
+        double room = budget;            // cost the current gang can still take
+        part_rows = 0;
+        for (const Str &st_ : order) {
+            const Segment &s = segs[st_.seg];
+            const int rows = s.nq * G;
+            if (part_rows > INT_MAX - (int64_t)rows * Hkv * (n_gangs + 1)) return SPORK_ERR_INVALID;
+            const int seg_base = (int)part_rows;   // partial row of (split sp, head h, row i) = base + (sp * Hkv + h) * rows + i
+            int nsplit = 0, done = 0;              // pieces so far, tiles of the segment already assigned
+            while (done < st_.tiles) {
+                const int left = st_.tiles - done;
+                int take;
+                if (gang == n_gangs - 1) {
+                    take = left;         // the last gang takes what remains
+                } else {
+                    take = (int)std::min<double>(left, std::floor(room - c0));
+                    if (take < std::min(left, MIN_CHUNK_TILES)) {   // no room for a useful piece: next gang
+                        ++gang;
+                        room = budget;
+                        continue;
+                    }
+                    if (left - take > 0 && left - take < MIN_CHUNK_TILES) take = left;   // no crumbs
                 }
+                const int t0 = s.tok0 + done * TILE_TOKENS;
+                const int t1 = std::min(s.tok1, t0 + take * TILE_TOKENS);
+                for (int h = 0; h < Hkv; ++h)
+                    per_cta[gang * Hkv + h].push_back(make_item(s, h, 0, t0, t1, seg_base + (nsplit * Hkv + h) * rows));
+                nsplit++;
+                done += take;
+                room -= take + c0;
+            }
+            for (int h = 0; h < Hkv; ++h)
+                streams[(size_t)st_.seg * Hkv + h] = StreamDesc{seg_base + h * rows, nsplit, Hkv * rows, 0};
+            part_rows += (int64_t)nsplit * Hkv * rows;
+        }
+        cta_ptr_umma.assign(G_ + 1, 0);
+        for (int b2 = 0; b2 < G_; ++b2) {
+            cta_ptr_umma[b2 + 1] = cta_ptr_umma[b2] + (int)per_cta[b2].size();
+            items_umma.insert(items_umma.end(), per_cta[b2].begin(), per_cta[b2].end());
+        }
+        chunk_tiles = (int)budget;
+        cta_ptr.assign(1, 0);
+        cta_ptr_umma2.assign(1, 0);
+    } else {
+        // ---- equal chunks per segment, items longest first, LPT onto each kernel's CTAs ----
+        items.reserve(n_items);
+        for (size_t si = 0; si < segs.size(); ++si) {
+            const Segment &s = segs[si];
+            const int rows = s.nq * G;
+            for (int h = 0; h < Hkv; ++h)
+                streams[si * Hkv + h] = StreamDesc{s.part_base + h * rows, s.nsplit, s.nq * Hq, 0};
+            std::vector<WorkItem> &dst = s.kind == 2 ? items_umma2 : (s.kind == 1 ? items_umma : items);
+            for (int sp = 0; sp < s.nsplit; ++sp) {
+                int t0 = s.tok0 + sp * s.chunk_tiles * TILE_TOKENS;
+                int t1 = std::min(s.tok1, t0 + s.chunk_tiles * TILE_TOKENS);
+                for (int h = 0; h < Hkv; ++h)
+                    for (int rb = 0; rb < rows; rb += s.row_block)
+                        dst.push_back(make_item(s, h, rb, t0, t1, s.part_base + sp * s.nq * Hq + h * rows + rb));
+            }
+        }
+        const int g0_ = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
+        if (mma) {
+            schedule(items, g0_, cta_ptr);
+            schedule(items_umma, (int)std::min<size_t>(items_umma.size(), (size_t)grid_cap_umma), cta_ptr_umma);
+            schedule(items_umma2, (int)std::min<size_t>(items_umma2.size(), (size_t)grid_cap_umma2), cta_ptr_umma2);
+        } else {
+            std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
+                return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
+            });
+            cta_ptr.assign(g0_ + 1, 0);
+            cta_ptr_umma.assign(1, 0);
+            cta_ptr_umma2.assign(1, 0);
         }
     }
-    const int grid = (int)std::min<size_t>(items.size(), (size_t)grid_cap);
-    const int grid_umma = (int)std::min<size_t>(items_umma.size(), (size_t)grid_cap_umma);
-    const int grid_umma2 = (int)std::min<size_t>(items_umma2.size(), (size_t)grid_cap_umma2);
-    std::vector<int32_t> cta_ptr, cta_ptr_umma, cta_ptr_umma2;
-    if (mma) {
-        schedule(items, grid, cta_ptr);
-        schedule(items_umma, grid_umma, cta_ptr_umma);
-        schedule(items_umma2, grid_umma2, cta_ptr_umma2);
-    } else {
-        std::stable_sort(items.begin(), items.end(), [](const WorkItem &a, const WorkItem &b) {
-            return (a.tok1 - a.tok0) > (b.tok1 - b.tok0);
-        });
-        cta_ptr.assign(grid + 1, 0);
-        cta_ptr_umma.assign(1, 0);
-        cta_ptr_umma2.assign(1, 0);
-    }
+    const int grid = (int)cta_ptr.size() - 1;
+    const int grid_umma = (int)cta_ptr_umma.size() - 1;
+    const int grid_umma2 = (int)cta_ptr_umma2.size() - 1;
     const int n_items_mma = (int)items.size();
     items.insert(items.end(), items_umma.begin(), items_umma.end());
     items.insert(items.end(), items_umma2.begin(), items_umma2.end());
@@ -391,23 +451,28 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     int rc = devbuf_reserve(&P.items, ib + 64, st);
     if (rc == SPORK_OK) rc = devbuf_reserve(&P.qdesc, qb + 64, st);
     if (rc == SPORK_OK) rc = devbuf_reserve(&P.cta_ptr, cb + 64, st);
+    const size_t sb = streams.size() * sizeof(StreamDesc);
+    if (rc == SPORK_OK) rc = devbuf_reserve(&P.streams, sb + 64, st);
 
     if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_o, (size_t)part_rows * c->cfg.head_dim * 4 + 64, st);
     if (rc == SPORK_OK) rc = devbuf_reserve(&c->ws_lse, (size_t)part_rows * 4 + 64, st);
     if (rc != SPORK_OK) return rc;
     if (ib + qb) {
         StageSlot *slot;
-        rc = stage_acquire(c, ib + qb + cb, &slot);
+        rc = stage_acquire(c, ib + qb + cb + sb, &slot);
         if (rc != SPORK_OK) return rc;
         if (ib) memcpy(slot->h, items.data(), ib);
         if (qb) memcpy((char *)slot->h + ib, qd.data(), qb);
         memcpy((char *)slot->h + ib + qb, cta_ptr.data(), cb);
-        rc = stage_commit(c, slot, ib + qb + cb, st);
+        if (sb) memcpy((char *)slot->h + ib + qb + cb, streams.data(), sb);
+        rc = stage_commit(c, slot, ib + qb + cb + sb, st);
         if (rc != SPORK_OK) return rc;
         if (ib) SPORK_CUDA(cudaMemcpyAsync(P.items.p, slot->d, ib, cudaMemcpyDeviceToDevice, st));
         if (qb)
             SPORK_CUDA(cudaMemcpyAsync(P.qdesc.p, (char *)slot->d + ib, qb, cudaMemcpyDeviceToDevice, st));
         SPORK_CUDA(cudaMemcpyAsync(P.cta_ptr.p, (char *)slot->d + ib + qb, cb, cudaMemcpyDeviceToDevice, st));
+        if (sb)
+            SPORK_CUDA(cudaMemcpyAsync(P.streams.p, (char *)slot->d + ib + qb + cb, sb, cudaMemcpyDeviceToDevice, st));
         rc = stage_done(c, slot, st);
         if (rc != SPORK_OK) return rc;
     }
@@ -434,6 +499,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     P.info.chunk_tokens = chunk_tiles * TILE_TOKENS;
     P.info.kernel = !mma ? 0 : (P.info.n_umma_items == 0 ? 1 : (P.n_items == 0 ? 2 : 3));
     P.info.plan_cached = 0;
+    P.info.stream_k = stream_k ? 1 : 0;
     P.info.unique_tokens = unique_tokens;
     P.info.naive_tokens = naive_tokens;
     P.info.partial_rows = part_rows;

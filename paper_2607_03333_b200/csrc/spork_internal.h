@@ -34,14 +34,20 @@ struct WorkItem {
 };
 static_assert(sizeof(WorkItem) == 48, "WorkItem layout");
 
-// Per q row: where its partials live.  Partial row index of (split s, head h):
-//   base + s * stride + (h / G) * nq * G + qi * G + h % G
-struct QRowDesc {
-    int32_t pre_base, pre_nsplit, pre_stride, pre_nq, pre_qi;
-    int32_t suf_base, suf_nsplit, suf_stride, suf_nq, suf_qi;
-    int32_t pad[2];
+// A stream = (segment, kv head): the partials of its rows.  Partial row index of
+// (split s, row i of the stream) = part_base + s * stride + i, rows ordered (q row, GQA head).
+// Different kv heads of one segment may be cut at different places (stream-K schedule).
+struct StreamDesc {
+    int32_t part_base, nsplit, stride, pad;
 };
-static_assert(sizeof(QRowDesc) == 48, "QRowDesc layout");
+static_assert(sizeof(StreamDesc) == 16, "StreamDesc layout");
+
+// Per q row: its shared-prefix stream and its private stream of kv head 0 (-1: none; kv head h
+// is stream + h) and the row's offset q_index * G inside them.
+struct QRowDesc {
+    int32_t pre_stream, pre_off, suf_stream, suf_off;
+};
+static_assert(sizeof(QRowDesc) == 16, "QRowDesc layout");
 
 // ---------------------------------------------------------------------------
 // staging ring: pinned host + device scratch for per-call descriptors
@@ -70,7 +76,7 @@ struct Plan {
     uint64_t shared_epoch = 0;
     std::vector<int32_t> shared_key_indptr, shared_key_ids;
     // device copies
-    DevBuf items, qdesc;
+    DevBuf items, qdesc, streams;
     // items = [n_items of the mma.sync / simt path][n_items_umma of the tcgen05 kernel, <= 128 rows]
     //         [n_items_umma2 of the two-pipe tcgen05 kernel, <= 256 rows];
     // cta_ptr = int32[grid + 1], int32[grid_umma + 1], int32[grid_umma2 + 1]: CTA b of a kernel
@@ -126,6 +132,7 @@ struct spork_ctx {
     cudaEvent_t plan_ev;
     bool plan_ev_pending;
     int timing = 0;
+    int stream_k = 1;             // equal-work contiguous schedule when every segment is one row block
     int two_pipe = 0;             // segments of > 128 rows: 0 default kernel, 1 two-pipe, 2 split-row kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};

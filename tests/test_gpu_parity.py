@@ -128,6 +128,15 @@ def test_small_bf16_decode(cfg, path):
     check_attn(out, lse, out_ref, lse_ref, "bf16", cfg.name)
     info = spk.last_plan()
     _check_kernel(info, path)
+    if path in ("auto", "tcgen05"):
+        # every segment is one row block -> stream-K schedule; the chunked LPT schedule gives the same
+        # result up to the rounding of a different split
+        assert info["stream_k"] == 1
+        spk.set_stream_k(False)
+        out_c, lse_c = spk.decode_attn(wl.group_indptr(), ids, q)
+        assert spk.last_plan()["stream_k"] == 0
+        check_attn(out_c, lse_c, out_ref, lse_ref, "bf16", cfg.name + " chunked schedule")
+        spk.set_stream_k(True)
     # an unaligned fork point duplicates the tail page: those tokens are private copies
     dup = cfg.n_groups * (cfg.group_size - 1) * (cfg.prefix_len % 16)
     assert info["unique_tokens"] == wl.unique_tokens() + dup
