@@ -167,16 +167,17 @@ def run_reference(args, cfg, name, wl):
     step, frac, cores, sample = oracle_sample(cfg, wl, args.ref_groups)
     for _ in range(max(0, min(args.warmup, 1))):
         step()
+    steps = min(args.steps, 20)            # a CPU step takes 0.05 .. 20 s: keep the run bounded
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
-    dt = (time.perf_counter() - t0) / args.steps
+    dt = (time.perf_counter() - t0) / steps
     full = dt / frac                       # time one whole step would take, scaled by flops
     ub = wl.unique_kv_bytes()
     val = ub / full / 1e9
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True,
+        "steps": steps, "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": name, "sample": sample, "sample_seconds_per_step": dt},
         "cpu_baseline": {"value": val, "unit": "GB/s", "cores": cores, "kind": "oracle", "sample": sample},
@@ -264,15 +265,16 @@ def run_ours(args, cfg, name, wl):
         torch.cuda.synchronize()
         return [a.elapsed_time(b) for a, b in evs]
 
+    # nvidia-smi samples every 100 ms: the sampler runs from the warm-up to the end of the e2e pass
+    # (the GPU is under the same load throughout), the timed region lies inside that window
+    sampler = ClockSampler(local)
+    sampler.start()
     for _ in range(max(args.warmup, 3)):
         flush_l2()
         step()
     barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
     ms = timed(args.steps)
     barrier()
-    clocks = sampler.stop()
     total_ms = float(sum(ms))
     if world > 1:
         t = torch.tensor([total_ms], device=device, dtype=torch.float64)
@@ -359,6 +361,7 @@ def run_ours(args, cfg, name, wl):
         o = oh.numpy()
         assert np.all(np.isfinite(o))
 
+    clocks = sampler.stop()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -411,7 +414,7 @@ def run_ours(args, cfg, name, wl):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "churn"])
     ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
@@ -429,7 +432,7 @@ def main():
     cfg, name = pick_config(args)
     wl = synth.Workload(cfg)
     if args.ref_groups <= 0:
-        args.ref_groups = {"2": 8, "3": 4, "4": 1, "5": 2, "churn": 1}[args.config]
+        args.ref_groups = {"2": 16, "3": 4, "4": 1, "5": 2, "churn": 1}[args.config]
     if args.impl == "reference":
         if int(os.environ.get("RANK", "0")) == 0:
             run_reference(args, cfg, name, wl)

@@ -148,6 +148,20 @@ class Oracle:
         s, nl = _i32(seq_ids), _i32(new_len)
         return self._chk(lib().oracle_truncate(self._h, len(s), _p(s), _p(nl)), check)
 
+    # ---- partial-token accept ---------------------------------
+    def accept(self, seq_ids, q_indptr, draft_tokens, target_tokens, check: bool = True):
+        """PAPER.md:236-237 (section 4.3): the engine "verifies the draft ... the first k matching tokens
+        are accepted".  Sequence i holds k_i = q_indptr[i+1] - q_indptr[i] drafts as its last k_i tokens;
+        target_tokens[j] is the target model's greedy token at draft position j.  accept_len_i = the
+        number of leading positions with draft == target; the rejected drafts' KV is dropped:
+        truncate(seq_i, len_i - (k_i - accept_len_i)).  Returns (rc, accept_len[n])."""
+        acc = accept_len(q_indptr, draft_tokens, target_tokens)
+        qi = np.asarray(q_indptr, dtype=np.int64)
+        k = qi[1:] - qi[:-1]
+        new_len = np.array([self.export_seq(int(s))[0] for s in seq_ids], dtype=np.int64) - (k - acc)
+        rc = self.truncate(seq_ids, new_len.astype(np.int32), check)
+        return rc, acc
+
     # ---- export -------------------------------------------------------------
     def export_seq(self, seq: int):
         """(len, table[ceil(len/ps)]); len = -1 if the slot is not live."""
@@ -230,3 +244,20 @@ def attend_dense(dtype: str, scale: float, q_row: np.ndarray, K: np.ndarray, V: 
     if rc != OK:
         raise OracleError(rc)
     return out, float(lse[0])
+
+
+def accept_len(q_indptr, draft_tokens, target_tokens) -> np.ndarray:
+    """Longest greedy-matching prefix per sequence, written out position by
+    position: walk the drafts of sequence i from the first; stop at the first mismatch."""
+    qi = np.asarray(q_indptr, dtype=np.int64)
+    d = np.asarray(draft_tokens)
+    t = np.asarray(target_tokens)
+    out = np.zeros(len(qi) - 1, dtype=np.int32)
+    for i in range(len(qi) - 1):
+        a = 0
+        for j in range(int(qi[i]), int(qi[i + 1])):
+            if int(d[j]) != int(t[j]):
+                break
+            a += 1
+        out[i] = a
+    return out
