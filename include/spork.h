@@ -222,6 +222,24 @@ int spork_set_timing(spork_ctx *ctx, int enable);
 int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
 
 /*
+ * Partial-token accept + rollback (section 4.3: "the first k matching tokens are
+ * accepted").  Sequence seq_ids[i] holds k_i = q_indptr[i+1] - q_indptr[i]
+ * draft tokens as its LAST k_i tokens (appended before spork_verify_attn).  draft_tokens and
+ * target_tokens are DEVICE int32 arrays of sum k_i entries, ragged by q_indptr: the drafts, and the
+ * target model's greedy token at each draft position (computed by the caller's LM head from the
+ * verify output; not part of this library).  For every sequence: accept_len_i = number of leading
+ * positions with draft == target (one warp per sequence); the rejected drafts' KV is rolled back as
+ * spork_truncate(seq_i, len_i - (k_i - accept_len_i)) does (whole pages beyond the new length are
+ * freed).  accept_len_out: HOST int32[n], written before return.  seq_ids, q_indptr: host, read
+ * before return.  Synchronises `stream` once (the host mirrors lengths).  Errors: SPORK_ERR_INVALID
+ * (k_i < 1, k_i > len_i, null pointers), SPORK_ERR_INVALID_SEQ, SPORK_ERR_SHARED as for
+ * spork_truncate; on a validation error nothing changes.
+ */
+int spork_accept(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t *q_indptr,
+                 const int32_t *draft_tokens, const int32_t *target_tokens, int32_t *accept_len_out,
+                 void *stream);
+
+/*
  * Tuning knob of the planner (bf16, D = 128 contexts only): a segment -- a fork group's shared
  * prefix or one sequence's private tail -- whose query rows x GQA heads per KV head number at
  * least `min_rows` is run by the tcgen05 (TMEM) kernel in row blocks of 128, the others by the

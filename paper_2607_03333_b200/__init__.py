@@ -32,7 +32,7 @@ ABI_SYMBOLS = [
     "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
-    "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
+    "spork_accept", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
 ]
 
 
@@ -90,6 +90,7 @@ def load(build_if_missing: bool = True):
         "spork_status": ([P], I),
         "spork_last_plan": ([P, P], I),
         "spork_last_launches": ([P], I),
+        "spork_accept": ([P, I, P, P, P, P, P, P], I),
         "spork_set_timing": ([P, I], I),
         "spork_set_tensor_path_min_rows": ([P, I], I),
         "spork_set_two_pipe": ([P, I], I),
@@ -223,6 +224,19 @@ class Spork:
     def truncate(self, seq_ids, new_len, check: bool = True) -> int:
         s, nl = _i32(seq_ids), _i32(new_len)
         return self._chk(self.lib.spork_truncate(self._h, len(s), _p(s), _p(nl), self._st), check)
+
+    def accept(self, seq_ids, q_indptr, draft_tokens, target_tokens, check: bool = True):
+        """Longest greedy-matching prefix per sequence + rollback of the rejected drafts.
+        draft_tokens / target_tokens: device int32 tensors (or numpy arrays).  Returns (rc, accept_len)."""
+        torch = self.torch
+        s, qi = _i32(seq_ids), _i32(q_indptr)
+        d = draft_tokens if hasattr(draft_tokens, "data_ptr") else self._dev(np.asarray(draft_tokens, dtype=np.int32))
+        t = target_tokens if hasattr(target_tokens, "data_ptr") else self._dev(np.asarray(target_tokens, dtype=np.int32))
+        assert d.dtype == torch.int32 and t.dtype == torch.int32
+        acc = np.zeros(len(s), np.int32)
+        rc = self._chk(self.lib.spork_accept(self._h, len(s), _p(s), _p(qi), C.c_void_p(d.data_ptr()),
+                                             C.c_void_p(t.data_ptr()), _p(acc), self._st), check)
+        return rc, acc
 
     # ---- attention ------------------------------------------------------------
     def decode_attn(self, group_indptr, seq_ids, q, out=None, lse=None, check: bool = True):

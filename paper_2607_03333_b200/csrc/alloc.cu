@@ -567,3 +567,73 @@ extern "C" int spork_truncate(spork_ctx *c, int n, const int32_t *seq_ids, const
     if (n == 0) return SPORK_OK;
     return drop_common(c, n, seq_ids, new_len, (cudaStream_t)stream);
 }
+
+// ---------------------------------------------------------------------------
+// partial-token accept
+// ---------------------------------------------------------------------------
+namespace {
+
+// one warp per sequence: index of the first draft position whose token differs from the target's
+__global__ void __launch_bounds__(128) accept_len_kernel(const int32_t *__restrict__ q_indptr,
+                                                         const int32_t *__restrict__ draft,
+                                                         const int32_t *__restrict__ target, int n,
+                                                         int32_t *__restrict__ accept_len) {
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n) return;
+    const int b = q_indptr[w], e = q_indptr[w + 1];
+    int first = e - b;
+    for (int j0 = b; j0 < e; j0 += 32) {
+        const int j = j0 + lane;
+        const bool mismatch = j < e && draft[j] != target[j];
+        const unsigned m = __ballot_sync(0xffffffffu, mismatch);
+        if (m) {
+            first = j0 - b + __ffs(m) - 1;
+            break;
+        }
+    }
+    if (lane == 0) accept_len[w] = first;
+}
+
+}  // namespace
+
+extern "C" int spork_accept(spork_ctx *c, int n, const int32_t *seq_ids, const int32_t *q_indptr,
+                            const int32_t *draft_tokens, const int32_t *target_tokens,
+                            int32_t *accept_len_out, void *stream) {
+    if (!c || n < 0) return SPORK_ERR_INVALID;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    if (!seq_ids || !q_indptr || !draft_tokens || !target_tokens || !accept_len_out || q_indptr[0] != 0)
+        return SPORK_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int i = 0; i < n; ++i) {
+        const int s = seq_ids[i], k = q_indptr[i + 1] - q_indptr[i];
+        if (s < 0 || s >= c->cfg.max_seqs || !c->h_live[s]) return SPORK_ERR_INVALID_SEQ;
+        if (k < 1 || k > c->h_len[s]) return SPORK_ERR_INVALID;
+    }
+    // q_indptr -> device, accept lengths <- device through one staging slot (the host needs the
+    // lengths to mirror len[] anyway: this is the call's one documented synchronisation)
+    const size_t ib = 4 * (size_t)(n + 1), ob = 4 * (size_t)n;
+    StageSlot *slot;
+    int rc = stage_acquire(c, ib + ob, &slot);
+    if (rc != SPORK_OK) return rc;
+    memcpy(slot->h, q_indptr, ib);
+    rc = stage_commit(c, slot, ib, st);
+    if (rc != SPORK_OK) return rc;
+    int32_t *d_out = (int32_t *)((char *)slot->d + ib);
+    accept_len_kernel<<<ceil_div(n, 4), 128, 0, st>>>((const int32_t *)slot->d, draft_tokens, target_tokens, n,
+                                                      d_out);
+    SPORK_CUDA(cudaGetLastError());
+    SPORK_CUDA(cudaMemcpyAsync(accept_len_out, d_out, ob, cudaMemcpyDeviceToHost, st));
+    SPORK_CUDA(cudaStreamSynchronize(st));
+    rc = stage_done(c, slot, st);
+    if (rc != SPORK_OK) return rc;
+    std::vector<int32_t> new_len(n);
+    for (int i = 0; i < n; ++i) {
+        const int k = q_indptr[i + 1] - q_indptr[i];
+        if (accept_len_out[i] < 0 || accept_len_out[i] > k) return SPORK_ERR_CUDA;
+        new_len[i] = c->h_len[seq_ids[i]] - (k - accept_len_out[i]);
+    }
+    rc = drop_common(c, n, seq_ids, new_len.data(), st);
+    c->last_launches++;     // + accept_len_kernel
+    return rc;
+}
