@@ -499,26 +499,28 @@ attn_umma_kernel(const UParams P) {
                 }
                 const float mu = m_used == -INFINITY ? 0.f : m_used;
                 uint32_t p[32];
-                float sum0 = 0.f, sum1 = 0.f, rs0 = 0.f, rs1 = 0.f;
+                // packed fp32 pairs for the scale, the exact sum and the sum of the rounded weights
+                float se0 = 0.f, se1 = 0.f, se2 = 0.f, se3 = 0.f, sr0 = 0.f, sr1 = 0.f, sr2 = 0.f, sr3 = 0.f;
+                const float nmu = -mu;
 #pragma unroll
                 for (int t = 0; t < 16; ++t) {
-                    const float a0 = ex2(fmaf(__uint_as_float(s0[2 * t]), P.scale_log2, -mu));
-                    const float a1 = ex2(fmaf(__uint_as_float(s0[2 * t + 1]), P.scale_log2, -mu));
-                    const float c0 = ex2(fmaf(__uint_as_float(s1[2 * t]), P.scale_log2, -mu));
-                    const float c1 = ex2(fmaf(__uint_as_float(s1[2 * t + 1]), P.scale_log2, -mu));
+                    float x0, x1, y0, y1;
+                    ffma2(x0, x1, __uint_as_float(s0[2 * t]), __uint_as_float(s0[2 * t + 1]), P.scale_log2, nmu);
+                    ffma2(y0, y1, __uint_as_float(s1[2 * t]), __uint_as_float(s1[2 * t + 1]), P.scale_log2, nmu);
+                    const float a0 = ex2(x0), a1 = ex2(x1), c0 = ex2(y0), c1 = ex2(y1);
                     p[t] = pack_bf16(a0, a1);
                     p[16 + t] = pack_bf16(c0, c1);
                     // o is normalised by the sum of the ROUNDED weights the tensor core uses, so that
                     // o = sum(p v) / sum(p) stays a true weighted mean (a one-hot row returns V exactly
                     // even when the running max is stale and p is not a power of two); lse keeps the
                     // exact sum
-                    sum0 += a0 + a1;
-                    sum1 += c0 + c1;
-                    rs0 += __uint_as_float(p[t] << 16) + __uint_as_float(p[t] & 0xffff0000u);
-                    rs1 += __uint_as_float(p[16 + t] << 16) + __uint_as_float(p[16 + t] & 0xffff0000u);
+                    fadd2(se0, se1, a0, a1);
+                    fadd2(se2, se3, c0, c1);
+                    fadd2(sr0, sr1, __uint_as_float(p[t] << 16), __uint_as_float(p[t] & 0xffff0000u));
+                    fadd2(sr2, sr3, __uint_as_float(p[16 + t] << 16), __uint_as_float(p[16 + t] & 0xffff0000u));
                 }
-                l += sum0 + sum1;
-                lr += rs0 + rs1;
+                l += (se0 + se1) + (se2 + se3);
+                lr += (sr0 + sr1) + (sr2 + sr3);
                 tmem_st32(tS, p);
                 tmem_wait_st();
                 if ((nv & (PS - 1)) && w == 0 && lg == 0) {
