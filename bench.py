@@ -187,6 +187,22 @@ def run_reference(args, cfg, name, wl):
     print(json.dumps(line))
 
 
+def max_over_ranks(x: float, device, world: int) -> float:
+    """Replicas only: the step time of an N-replica run is the slowest rank's."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(unique_bytes: int, ms_step: float, world: int) -> float:
+    """Whole-job GB/s of `world` independent replicas that each moved `unique_bytes` in `ms_step`."""
+    return world * unique_bytes / (ms_step * 1e-3) / 1e9
+
+
 # ---------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------
@@ -275,11 +291,7 @@ def run_ours(args, cfg, name, wl):
     barrier()
     ms = timed(args.steps)
     barrier()
-    total_ms = float(sum(ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(sum(ms)), device, world)
     ms_step = total_ms / args.steps
 
     info = spk.last_plan() if not churn else {}
@@ -349,12 +361,8 @@ def run_ours(args, cfg, name, wl):
             t0 = time.perf_counter()
             e2e_step()
             tt.append(time.perf_counter() - t0)
-        e_ms = float(np.mean(tt)) * 1e3
-        if world > 1:
-            t = torch.tensor([e_ms], device=device, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_ms = float(t.item())
-        e2e = {"value": world * ub / (e_ms * 1e-3) / 1e9, "unit": "GB/s", "ms_per_step": e_ms,
+        e_ms = max_over_ranks(float(np.mean(tt)) * 1e3, device, world)
+        e2e = {"value": aggregate_value(ub, e_ms, world), "unit": "GB/s", "ms_per_step": e_ms,
                "h2d_bytes_per_step": int(qh.numel() * qh.element_size()),
                "d2h_bytes_per_step": int(oh.numel() * 4 + lh.numel() * 4)}
         # parity spot check of what was just timed (oracle, one sampled row)
@@ -379,7 +387,7 @@ def run_ours(args, cfg, name, wl):
     if churn:
         value, unit, metric = 10000 / (ms_step * 1e-3), "forks/s", "fork_release_churn"
     else:
-        value, unit, metric = world * ub / (ms_step * 1e-3) / 1e9, "GB/s", METRIC
+        value, unit, metric = aggregate_value(ub, ms_step, world), "GB/s", METRIC
     line = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
