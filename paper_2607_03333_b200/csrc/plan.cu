@@ -58,6 +58,9 @@ constexpr int ROW_BLOCK = 64;
 constexpr int ROW_BLOCK_UMMA = 128;
 constexpr float ITEM_FIXED_COST = 1.5f;        // per-item overhead in 64-token-tile times
 constexpr float ITEM_FIXED_COST_UMMA = 4.f;    // ... of the tcgen05 kernel (32 KiB of Q, 64 KiB of partials)
+// ... of a tcgen05 item in the chunked schedule, which serves the many-row (compute-heavy) verify
+// plans (sweep of the chunk length on config 4, k = 16: 630 / 587 / 650 / 669 us at 1 / 2 / 3 / 4 splits)
+constexpr float ITEM_FIXED_COST_UMMA_CHUNKED = 8.f;
 
 struct Segment {
     int table_seq, tok0, tok1;  // token range
@@ -262,7 +265,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             for (int sp = 0; sp < s.nsplit; ++sp) {
                 // a two-pipe CTA has the SM to itself: a tile takes it half the time of a one-pipe CTA
                 const float t = ((float)std::min(s.chunk_tiles, tiles - sp * s.chunk_tiles) +
-                                 (kind ? ITEM_FIXED_COST_UMMA : ITEM_FIXED_COST)) *
+                                 (kind ? ITEM_FIXED_COST_UMMA_CHUNKED : ITEM_FIXED_COST)) *
                                 (kind == 2 && c->two_pipe == 1 ? 0.5f : 1.f);
                 cost.insert(cost.end(), (size_t)Hkv * n_rb, t);
             }
@@ -286,6 +289,8 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     size_t n_items = 0;
     {
         static const float mult[] = {1.f, 1.5f, 2.f, 3.f, 4.f, 6.f};
+        bool heavy = false;      // some tcgen05 segment has several row blocks
+        for (const Segment &sg : segs) heavy = heavy || (sg.kind != 0 && sg.nq * G > sg.row_block);
         double best = -1.0;
         int best_chunk = -1;
         const int row_bytes = c->cfg.head_dim * 4 + 4;
@@ -298,7 +303,12 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
             size_t ni;
             if (!split(ct, &pr, &ni)) continue;
             const double partial = 2.0 * (double)pr * row_bytes / tile_bytes / grid_cap;
-            const double est = makespan(0, grid_cap) + makespan(1, grid_cap_umma) + makespan(2, grid_cap_umma2) + partial;
+            double est = makespan(0, grid_cap) + makespan(1, grid_cap_umma) + makespan(2, grid_cap_umma2) + partial;
+            // Many-row verify plans are bound by the SMs, not by HBM: two co-resident CTAs speed each
+            // other up when one runs dry, which the per-CTA makespan does not see.  Measured on
+            // config 4 (k = 8, 16; sweep in DESIGN.md): 4.5 to 6 items per CTA is the sweet spot, so
+            // candidates outside it are handicapped.
+            if (heavy && (2 * ni < 9 * (size_t)grid_cap_umma || ni > 6 * (size_t)grid_cap_umma)) est *= 1.25;
             if (best < 0.0 || est < best) {
                 best = est;
                 best_chunk = ct;
