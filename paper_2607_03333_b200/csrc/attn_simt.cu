@@ -150,6 +150,7 @@ __global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__
                                                     const StreamDesc *__restrict__ streams, int n_qrows, int Hq,
                                                     int G, int D, const float *ws_o, const float *ws_lse,
                                                     float *__restrict__ out, float *__restrict__ lse) {
+    // one warp per (q row, q head): the most warps, for calls with few rows (decode)
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (w >= n_qrows * Hq) return;
     const int qrow = w / Hq, h = w % Hq;
@@ -157,6 +158,38 @@ __global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__
     const RowStreams rs = load_row_streams(streams, d, h / G);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     merge_row<NI>(rs, d, h % G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
+}
+
+template <int NI>
+__global__ void __launch_bounds__(128) merge_heads_kernel(const QRowDesc *__restrict__ qd,
+                                                          const StreamDesc *__restrict__ streams, int n_qrows,
+                                                          int Hq, int G, int D, const float *ws_o,
+                                                          const float *ws_lse, float *__restrict__ out,
+                                                          float *__restrict__ lse) {
+    // one warp per (q row, kv head): its G heads' partial rows are contiguous; for calls with many rows
+    // (verify, large decode batches), where bytes in flight per warp matter more than the warp count
+    const int Hkv = Hq / G;
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n_qrows * Hkv) return;
+    const int qrow = w / Hkv, kvh = w % Hkv;
+    const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
+    const RowStreams rs = load_row_streams(streams, d, kvh);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const size_t row0 = (size_t)qrow * Hq + (size_t)kvh * G;
+    constexpr int JB = NI == 1 ? 8 : 4;
+    int j = 0;
+    for (; j + JB <= G; j += JB)
+        merge_heads<NI, JB>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+    if (G - j >= 4 && JB > 4) {
+        merge_heads<NI, 4>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        j += 4;
+    }
+    if (G - j >= 2) {
+        merge_heads<NI, 2>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        j += 2;
+    }
+    for (; j < G; ++j)
+        merge_row<NI>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
 }
 
 }  // namespace
@@ -194,7 +227,10 @@ int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st) {
 int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_qrows == 0) return SPORK_OK;
-    const int warps = P.n_qrows * c->cfg.num_q_heads;
+    // enough (q row, kv head) pairs to fill the SMs: the grouped kernel (measured: verify k = 16 merge
+    // 60 -> 37 us, config 3 14 -> 12 us; config 2 / 5 with 256 / 512 pairs are faster per head)
+    const bool grouped = P.n_qrows * c->cfg.num_kv_heads >= 1024;
+    const int warps = P.n_qrows * (grouped ? c->cfg.num_kv_heads : c->cfg.num_q_heads);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(ceil_div(warps, 4));
     cfg.blockDim = dim3(128);
@@ -204,7 +240,9 @@ int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    SPORK_CUDA(cudaLaunchKernelEx(&cfg, c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>,
+    auto kern = grouped ? (c->cfg.head_dim <= 128 ? merge_heads_kernel<1> : merge_heads_kernel<2>)
+                        : (c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>);
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, kern,
                                   (const QRowDesc *)P.qdesc.p, (const StreamDesc *)P.streams.p, P.n_qrows,
                                   (int)c->cfg.num_q_heads, c->G, (int)c->cfg.head_dim,
                                   (const float *)c->ws_o.p, (const float *)c->ws_lse.p, out, lse));

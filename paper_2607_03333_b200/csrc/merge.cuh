@@ -97,4 +97,79 @@ __device__ __forceinline__ void merge_row(const RowStreams &rs, const QRowDesc &
     if (lane == 0) *lse_out = M + logf(W);
 }
 
+
+// The same combine for JB consecutive GQA heads of one (q row, kv head) at once -- their partial rows
+// are contiguous (JB x D floats per split), so one warp streams JB * 512 B per split with every load
+// of a split in flight: one descriptor fetch and JB times the memory-level parallelism per warp.
+// JB is a power of two <= 8; lane `e` of a batch owns the weight of (split e / JB, head e % JB).
+template <int NI, int JB>
+__device__ __forceinline__ void merge_heads(const RowStreams &rs, const QRowDesc &d, int j0, int D,
+                                            const float *ws_o, const float *ws_lse, float *out_rows,
+                                            float *lse_out, int lane) {
+    const StreamDesc &pre = rs.pre, &suf = rs.suf;
+    const int pre0 = pre.part_base + d.pre_off + j0;
+    const int suf0 = suf.part_base + d.suf_off + j0;
+    const int n = pre.nsplit + suf.nsplit;
+    auto part = [&](int s) -> size_t {          // partial row of (split s, head j0)
+        return s < pre.nsplit ? (size_t)pre0 + (size_t)s * pre.stride
+                              : (size_t)suf0 + (size_t)(s - pre.nsplit) * suf.stride;
+    };
+    constexpr int SB = 32 / JB;                 // splits per batch of 32 lanes
+    const int jj = lane % JB, sl = lane / JB;
+    // ---- row maxima ----
+    float M = -INFINITY;
+    for (int s = sl; s < n; s += SB) M = fmaxf(M, __ldcg(ws_lse + part(s) + jj));
+#pragma unroll
+    for (int o = JB; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));   // lanes of head jj
+    const int nv = D >> 2;
+    float4 acc[JB][NI];
+    float W[JB];
+#pragma unroll
+    for (int k = 0; k < JB; ++k) {
+        W[k] = 0.f;
+#pragma unroll
+        for (int i = 0; i < NI; ++i) acc[k][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    for (int s0 = 0; s0 < n; s0 += SB) {
+        const int s_mine = s0 + sl;
+        const float wl = (s_mine < n && M != -INFINITY) ? expf(__ldcg(ws_lse + part(s_mine) + jj) - M) : 0.f;
+        const int nb = min(SB, n - s0);
+        for (int sb = 0; sb < nb; ++sb) {
+            const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(s0 + sb) * D);
+            float4 v[JB][NI];
+#pragma unroll
+            for (int k = 0; k < JB; ++k)
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int c = lane + 32 * i;
+                    v[k][i] = c < nv ? __ldcg(po + (size_t)k * nv + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+#pragma unroll
+            for (int k = 0; k < JB; ++k) {
+                const float w = __shfl_sync(0xffffffffu, wl, sb * JB + k);
+                W[k] += w;
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    acc[k][i].x = fmaf(w, v[k][i].x, acc[k][i].x);
+                    acc[k][i].y = fmaf(w, v[k][i].y, acc[k][i].y);
+                    acc[k][i].z = fmaf(w, v[k][i].z, acc[k][i].z);
+                    acc[k][i].w = fmaf(w, v[k][i].w, acc[k][i].w);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < JB; ++k) {
+        const float inv = W[k] > 0.f ? 1.f / W[k] : 0.f;     // no partial / all empty: out = 0
+        float4 *o = reinterpret_cast<float4 *>(out_rows + (size_t)k * D);
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            const int c = lane + 32 * i;
+            if (c < nv) o[c] = make_float4(acc[k][i].x * inv, acc[k][i].y * inv, acc[k][i].z * inv, acc[k][i].w * inv);
+        }
+        const float Mk = __shfl_sync(0xffffffffu, M, k);     // lane k holds head k's maximum
+        if (lane == 0) lse_out[k] = W[k] > 0.f ? Mk + logf(W[k]) : -INFINITY;
+    }
+}
+
 }  // namespace spork
