@@ -261,3 +261,24 @@ def accept_len(q_indptr, draft_tokens, target_tokens) -> np.ndarray:
             a += 1
         out[i] = a
     return out
+
+
+def confidence(logits, span_indptr) -> np.ndarray:
+    """D2 confidence score, Eq. 2: c = min_{i=2..L} exp(l_i), l_i the
+    log-probability of the TOP-1 token at position i of the tool-name span.  logits: [n_pos][V], the
+    spans are consecutive row ranges [span_indptr[s], span_indptr[s+1]); the first row of a span is
+    skipped (i starts at 2: "the opening quote is always high-probability boilerplate"); a span of
+    L <= 1 rows has an empty minimum, read as 1 (reading A-23).  fp64, the plain definition:
+    l_i = x_max - ln sum_v exp(x_v)."""
+    x = np.asarray(logits, dtype=np.float64)
+    sp = np.asarray(span_indptr, dtype=np.int64)
+    out = np.ones(len(sp) - 1, dtype=np.float64)
+    for s in range(len(sp) - 1):
+        c = 1.0
+        for i in range(int(sp[s]) + 1, int(sp[s + 1])):
+            row = x[i]
+            m = float(row.max())
+            lse = m + np.log(np.sum(np.exp(row - m)))
+            c = min(c, float(np.exp(m - lse)))
+        out[s] = c
+    return out
