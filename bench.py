@@ -1,13 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line per run (the driver's contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|churn] [--k 4|8|16]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|churn|d2] [--k 4|8|16]
                     [--impl reference]
 
 A step = one pass of the hot path over one batch of synthetic input:
   configs 2/3/5  one spork_decode_attn call (plan lookup, cascade decode kernel, merge kernel)
   config 4       one spork_verify_attn call with k drafts per sequence
   churn          one spork_fork of 10,000 children + one spork_release of them (config 5)
+  d2             one spork_confidence call: Eq. 2 over 256 probe spans of Qwen3-vocabulary logits
 Default workload: BASELINE.json configs[1] (Qwen3-4B shape, 16 fork groups of 2, prefix 4096).
 Inputs are seeded synthetic (synth/), resident in HBM before the timed region; L2 is flushed
 between timed iterations.  `value` = unique KV bytes / step time (GB/s); config 4 also reports
@@ -424,12 +425,135 @@ def run_ours(args, cfg, name, wl):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------
+# D2 confidence: a stream over probe logits
+# ---------------------------------------------------------------------------
+D2_SPANS, D2_VOCAB = 256, 151936       # 256 probes in flight, Qwen3 vocabulary
+
+
+def run_d2(args):
+    import torch
+    import paper_2607_03333_b200 as sp
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    x, spn = synth.probe_logits(D2_SPANS, D2_VOCAB, seed=0)
+    rows_read = int(np.maximum(np.diff(spn) - 1, 0).sum())
+    alg_bytes = rows_read * D2_VOCAB * 4
+    name = "d2_confidence_qwen3_vocab"
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        import oracle
+        g = 16                              # spans in the oracle's bounded sample
+        t0 = time.perf_counter()
+        oracle.confidence(x[:spn[g]], spn[:g + 1])
+        dt = time.perf_counter() - t0
+        frac = float(np.maximum(np.diff(spn[:g + 1]) - 1, 0).sum()) / rows_read
+        val = alg_bytes / (dt / frac) / 1e9
+        sample = f"{g} of {D2_SPANS} spans, numpy fp64, 1 thread"
+        print(json.dumps({"impl": "reference", "metric": "d2_confidence_logits_bandwidth", "value": val,
+                          "unit": "GB/s", "n_gpus": args.gpus, "steps": 1, "warmup": 0,
+                          "ms_per_step": dt / frac * 1e3, "higher_is_better": True, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": name, "sample": sample},
+                          "cpu_baseline": {"value": val, "unit": "GB/s", "cores": 1, "kind": "oracle", "sample": sample},
+                          "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}))
+        return
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    device = f"cuda:{local}"
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    peaks = load_peaks()
+    spk = sp.Spork("f32", 4, 1, 64, 8, 2, 4, 0.125, device=device)
+    st = spk.stream
+    xd = spk._dev(x)
+    out = torch.empty((D2_SPANS,), dtype=torch.float32, device=device)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)
+    clean = torch.zeros(64 << 20, dtype=torch.int32, device=device)
+
+    def flush_l2():
+        with torch.cuda.stream(st):
+            flush.zero_()
+            clean.max()
+
+    def step():
+        spk.confidence(spn, xd, out)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        flush_l2()
+        step()
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in evs:
+        flush_l2()
+        a.record(st)
+        step()
+        b.record(st)
+    torch.cuda.synchronize()
+    ms_step = max_over_ranks(float(sum(a.elapsed_time(b) for a, b in evs)), device, world) / args.steps
+    # e2e: logits in pinned host memory, copied in every step; the scores copied back
+    xh = torch.from_numpy(x).pin_memory()
+    oh = torch.empty((D2_SPANS,), dtype=torch.float32).pin_memory()
+    tt = []
+    for _ in range(min(args.steps, 10)):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(st):
+            xd.copy_(xh, non_blocking=True)
+            step()
+            oh.copy_(out, non_blocking=True)
+        st.synchronize()
+        tt.append(time.perf_counter() - t0)
+    e_ms = max_over_ranks(float(np.mean(tt)) * 1e3, device, world)
+    clocks = sampler.stop()
+    if rank != 0:
+        return
+    import oracle
+    want = oracle.confidence(x[:spn[8]], spn[:9])
+    got = oh.numpy()[:8]
+    assert np.allclose(got, want, rtol=2e-5), "bench output does not match the oracle"
+    cpu = None
+    if not args.no_cpu_baseline:
+        g = 16
+        t0 = time.perf_counter()
+        oracle.confidence(x[:spn[g]], spn[:g + 1])
+        dt = time.perf_counter() - t0
+        frac = float(np.maximum(np.diff(spn[:g + 1]) - 1, 0).sum()) / rows_read
+        cpu = {"value": alg_bytes / (dt / frac) / 1e9, "unit": "GB/s", "cores": 1, "kind": "oracle",
+               "sample": f"{g} of {D2_SPANS} spans, numpy fp64, 1 thread", "sample_seconds": dt}
+    ach = alg_bytes / (ms_step * 1e-3) / 1e9
+    line = {"metric": "d2_confidence_logits_bandwidth", "value": aggregate_value(alg_bytes, ms_step, world),
+            "unit": "GB/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "us_per_step": ms_step * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": name, "spans": D2_SPANS, "vocab": D2_VOCAB, "rows_read": rows_read,
+                       "algorithmic_bytes": alg_bytes,
+                       "l2": "flushed between timed iterations (512 MiB write, then 256 MiB read)",
+                       "parallelism": "replicas only" if world > 1 else "1 gpu"},
+            "clocks": clocks, "gpu_launches": 2 * args.steps,
+            "roofline": {"bound": "hbm", "achieved": ach, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                         "frac": ach / float(peaks["hbm_gbs"]), "traffic": None,
+                         "kernel": "conf_partial_kernel+conf_span_kernel (whole call)",
+                         "peak_source": peaks["_source"], "algorithmic_bytes": alg_bytes},
+            "e2e": {"value": aggregate_value(alg_bytes, e_ms, world), "unit": "GB/s", "ms_per_step": e_ms,
+                    "h2d_bytes_per_step": int(x.nbytes), "d2h_bytes_per_step": int(4 * D2_SPANS)}}
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "churn"])
+    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "churn", "d2"])
     ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-groups", type=int, default=0,
@@ -442,6 +566,9 @@ def main():
                     help="planner knob: rows per KV head from which a segment runs on the tcgen05 kernel")
     ap.add_argument("--full-pool", action="store_true", help="config 5 on the 2^20-page pool")
     args = ap.parse_args()
+    if args.config == "d2":
+        run_d2(args)
+        return
     cfg, name = pick_config(args)
     wl = synth.Workload(cfg)
     if args.ref_groups <= 0:

@@ -240,6 +240,19 @@ int spork_accept(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t *q
                  void *stream);
 
 /*
+ * D2 confidence score (Eq. 2): for each of n_spans tool-name
+ * spans, c = min_{i=2..L} exp(l_i), l_i the log-probability of the TOP-1 token at position i, i.e.
+ * min_i 1 / sum_v exp(x_iv - max_v x_iv).  logits: DEVICE fp32 [n_pos][vocab], row-major, rows of span
+ * s are [span_indptr[s], span_indptr[s+1]) (span_indptr: HOST int32[n_spans + 1], starts at 0, read
+ * before return); the first row of a span is skipped (i starts at 2), a span of <= 1 rows gives 1.
+ * confidence_out: DEVICE fp32[n_spans].  Stream-ordered, no synchronisation.  The gate itself
+ * (c >= theta) is the caller's.  Errors: SPORK_ERR_INVALID (null pointers, vocab < 1,
+ * decreasing span_indptr).
+ */
+int spork_confidence(spork_ctx *ctx, int n_spans, const int32_t *span_indptr, const float *logits,
+                     int vocab, float *confidence_out, void *stream);
+
+/*
  * Tuning knob of the planner (bf16, D = 128 contexts only): a segment -- a fork group's shared
  * prefix or one sequence's private tail -- whose query rows x GQA heads per KV head number at
  * least `min_rows` is run by the tcgen05 (TMEM) kernel in row blocks of 128, the others by the

@@ -32,7 +32,7 @@ ABI_SYMBOLS = [
     "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
-    "spork_accept", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
+    "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
 ]
 
 
@@ -91,6 +91,7 @@ def load(build_if_missing: bool = True):
         "spork_last_plan": ([P, P], I),
         "spork_last_launches": ([P], I),
         "spork_accept": ([P, I, P, P, P, P, P, P], I),
+        "spork_confidence": ([P, I, P, P, I, P, P], I),
         "spork_set_timing": ([P, I], I),
         "spork_set_tensor_path_min_rows": ([P, I], I),
         "spork_set_two_pipe": ([P, I], I),
@@ -237,6 +238,20 @@ class Spork:
         rc = self._chk(self.lib.spork_accept(self._h, len(s), _p(s), _p(qi), C.c_void_p(d.data_ptr()),
                                              C.c_void_p(t.data_ptr()), _p(acc), self._st), check)
         return rc, acc
+
+    def confidence(self, span_indptr, logits, out=None, check: bool = True):
+        """Eq. 2 confidence per span.  logits: device fp32 tensor [n_pos][vocab] (or numpy).  Returns a
+        device fp32 tensor [n_spans]."""
+        torch = self.torch
+        sp = _i32(span_indptr)
+        x = logits if hasattr(logits, "data_ptr") else self._dev(np.asarray(logits, dtype=np.float32))
+        assert x.dtype == torch.float32 and x.is_contiguous()
+        n = len(sp) - 1
+        if out is None:
+            out = torch.empty((n,), dtype=torch.float32, device=self.device)
+        rc = self._chk(self.lib.spork_confidence(self._h, n, _p(sp), C.c_void_p(x.data_ptr()), int(x.shape[1]),
+                                                 C.c_void_p(out.data_ptr()), self._st), check)
+        return out if check else (rc, out)
 
     # ---- attention ------------------------------------------------------------
     def decode_attn(self, group_indptr, seq_ids, q, out=None, lse=None, check: bool = True):

@@ -173,7 +173,7 @@ extern "C" int spork_destroy(spork_ctx *c) {
         if (s.d) cudaFree(s.d);
         if (s.ev) cudaEventDestroy(s.ev);
     }
-    for (DevBuf *b : {&c->plan.items, &c->plan.qdesc, &c->plan.streams, &c->plan.cta_ptr, &c->ws_o, &c->ws_lse, &c->io_q, &c->io_out,
+    for (DevBuf *b : {&c->plan.items, &c->plan.qdesc, &c->plan.streams, &c->plan.cta_ptr, &c->ws_o, &c->ws_lse, &c->ws_conf, &c->conf_desc, &c->io_q, &c->io_out,
                       &c->io_lse})
         if (b->p) cudaFree(b->p);
     if (c->plan_ev) cudaEventDestroy(c->plan_ev);

@@ -127,6 +127,9 @@ struct spork_ctx {
     spork::Plan plan;
     spork::DevBuf ws_o, ws_lse;   // split-KV partials
     spork::DevBuf io_q, io_out, io_lse;  // device buffers of the *_host calls
+    spork::DevBuf ws_conf;               // per-(row, slice) partials of spork_confidence
+    spork::DevBuf conf_desc;             // its device descriptors, cached while the spans stay the same
+    std::vector<int32_t> conf_key;
     void *h_io = nullptr;         // pinned bounce (unused if caller memory is pinned)
     int last_launches;
     cudaEvent_t plan_ev;

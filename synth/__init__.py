@@ -300,3 +300,25 @@ def churn_parents(cfg_no: int, n_forks: int, live_ids: np.ndarray, index: int = 
     """Config 5 fork churn: parents drawn uniformly from the live sequences."""
     r = rng(cfg_no, T_CHURN, index)
     return np.asarray(live_ids, dtype=np.int32)[r.integers(0, len(live_ids), size=n_forks)]
+
+
+# ---------------------------------------------------------------------------
+# D2 confidence (SURVEY 8(f) NEXT-3): synthetic next-token logits of probe tool-name spans
+# ---------------------------------------------------------------------------
+T_LOGITS = 40
+
+
+def probe_logits(n_spans: int, vocab: int, seed: int = 0, max_len: int = 5):
+    """fp32 logits [n_pos][vocab] and span_indptr[n_spans + 1] for `n_spans` tool-name spans of
+    1..max_len generated tokens each ("typically 1-4 tokens" after the opening
+    quote, which is the span's first row).  Rows are N(0, 2^2) noise; one token per row is
+    lifted by U(0, 14) so that top-1 probabilities spread over (0, 1) as in Fig. 8
+    (PAPER.md:215-223).  Stand-in for real probe logits (no model weights here)."""
+    r = rng(0, T_LOGITS, seed)
+    lens = r.integers(1, max_len + 1, size=n_spans)
+    indptr = np.concatenate([[0], np.cumsum(lens)]).astype(np.int32)
+    n_pos = int(indptr[-1])
+    x = (2.0 * r.standard_normal((n_pos, vocab), dtype=np.float32)).astype(np.float32)
+    top = r.integers(0, vocab, size=n_pos)
+    x[np.arange(n_pos), top] += r.uniform(0.0, 14.0, size=n_pos).astype(np.float32)
+    return x, indptr
