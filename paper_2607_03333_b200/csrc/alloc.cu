@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <unordered_map>
 
 #include "spork_internal.h"
 
@@ -245,9 +246,14 @@ __global__ void __launch_bounds__(256) fork_refcount_kernel(const ParentDesc *__
 // ---- release / truncate ------------------------------------------------------
 struct DropDesc {
     int32_t seq, keep_pages, n_pages, new_len;
+    // release of several children of one fork (same parent, same call): their first agg_upto table
+    // entries are the same pages.  The first of them in the request subtracts the whole family's
+    // references at once (agg_mult = family size), the others skip those pages (agg_mult = 0):
+    // 10k releases of 128 families are 0.3 M atomics on the hot pages instead of 21.8 M.
+    int32_t agg_upto, agg_mult;
 };
 
-// one block per sequence: drop one reference from pages [keep_pages, n_pages)
+// one block per sequence: drop its references from pages [keep_pages, n_pages)
 __global__ void __launch_bounds__(256) drop_pages_kernel(const DropDesc *__restrict__ descs,
                                                          int32_t *table, int table_stride,
                                                          int32_t *len, int32_t *refcount,
@@ -258,13 +264,27 @@ __global__ void __launch_bounds__(256) drop_pages_kernel(const DropDesc *__restr
     __syncthreads();
     int32_t *row = table + (size_t)d.seq * table_stride;
     int freed = 0;
-    for (int j = d.keep_pages + threadIdx.x; j < d.n_pages; j += blockDim.x) {
-        int p = row[j];
-        row[j] = -1;
-        if (p < 0) { atomicExch(&counters[1], 1); continue; }   // consistency check
-        int old = atomicSub(&refcount[p], 1);
-        if (old == 1) ++freed;
-        if (old <= 0) atomicExch(&counters[1], 2);
+    // 4 table entries per thread are loaded before the first store / atomic (which the compiler must
+    // keep in order with later loads of the same array): one memory round trip per 1,024 pages
+    for (int j0 = d.keep_pages + threadIdx.x; j0 < d.n_pages; j0 += 4 * blockDim.x) {
+        int p[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u * blockDim.x;
+            p[u] = j < d.n_pages ? __ldcg(row + j) : -2;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u * blockDim.x;
+            if (p[u] == -2) continue;
+            row[j] = -1;
+            if (p[u] < 0) { atomicExch(&counters[1], 1); continue; }   // consistency check
+            const int mult = j < d.agg_upto ? d.agg_mult : 1;
+            if (mult == 0) continue;                                   // the family's leader drops these
+            int old = atomicSub(&refcount[p[u]], mult);
+            if (old == mult) ++freed;
+            if (old < mult) atomicExch(&counters[1], 2);
+        }
     }
     for (int o = 16; o; o >>= 1) freed += __shfl_down_sync(0xffffffffu, freed, o);
     if ((threadIdx.x & 31) == 0 && freed) atomicAdd(&s_freed, freed);
@@ -439,6 +459,7 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
     }
     for (int j = 0; j < n_par; ++j) pd[j].count = c->h_scratch[pd[j].parent];
     // children: lowest free slots in request order
+    c->fork_calls++;
     int tail = 0;
     for (int i = 0, s = 0; i < n; ++s) {
         if (c->h_live[s]) continue;
@@ -447,6 +468,8 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
         c->h_len[s] = L;
         c->h_shared_upto[s] = L / PS;
         c->h_shared_upto[p] = std::max(c->h_shared_upto[p], L / PS);
+        c->h_fork_key[s] = (c->fork_calls << 32) | (uint64_t)(p + 1);   // same call, same parent: same prefix
+        c->h_fork_nf[s] = L / PS;
         fd[i].parent = p;
         fd[i].child = s;
         fd[i].len = L;
@@ -511,10 +534,33 @@ static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_
         d[i].n_pages = pages_of(c->h_len[s]);
         d[i].new_len = new_len ? new_len[i] : 0;
         d[i].keep_pages = new_len ? pages_of(new_len[i]) : 0;
+        d[i].agg_upto = 0;
+        d[i].agg_mult = 1;
         // a partially filled kept tail page can only be shared below h_shared_upto
         if (new_len && (new_len[i] % PS) && new_len[i] / PS < c->h_shared_upto[s]) need_check = true;
     }
     if (host_err != SPORK_OK && !need_check) return host_err;
+    if (!new_len && n_ok > 1) {
+        // families: released children that still carry the same fork key (parent slot + fork call)
+        std::unordered_map<uint64_t, int> leader;     // key -> index of the family's first member
+        leader.reserve((size_t)n_ok);
+        for (int i = 0; i < n_ok; ++i) {
+            const int s = seq_ids[i];
+            const uint64_t key = c->h_fork_key[s];
+            const int nf = std::min(c->h_fork_nf[s], d[i].n_pages);
+            if (key == 0 || nf == 0) continue;
+            auto it = leader.find(key);
+            if (it == leader.end()) {
+                leader.emplace(key, i);
+                d[i].agg_upto = nf;
+                d[i].agg_mult = 1;
+            } else {
+                d[it->second].agg_mult++;
+                d[i].agg_upto = nf;
+                d[i].agg_mult = 0;
+            }
+        }
+    }
     rc = stage_commit(c, slot, sizeof(DropDesc) * (size_t)n_ok, st);
     if (rc != SPORK_OK) return rc;
     if (need_check) {
@@ -541,10 +587,12 @@ static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_
         if (new_len) {
             c->h_len[s] = new_len[i];
             c->h_shared_upto[s] = std::min(c->h_shared_upto[s], pages_of(new_len[i]));
+            c->h_fork_key[s] = 0;      // a rolled-back sequence no longer mirrors its siblings
         } else {
             c->h_len[s] = 0;
             c->h_live[s] = 0;
             c->h_shared_upto[s] = 0;
+            c->h_fork_key[s] = 0;
         }
     }
     if (!new_len) c->n_live -= n;

@@ -131,6 +131,8 @@ extern "C" int spork_create(const spork_config *cfg, void *k_pool, void *v_pool,
     c->h_len.assign(cfg->max_seqs, 0);
     c->h_live.assign(cfg->max_seqs, 0);
     c->h_shared_upto.assign(cfg->max_seqs, 0);
+    c->h_fork_key.assign(cfg->max_seqs, 0);
+    c->h_fork_nf.assign(cfg->max_seqs, 0);
     c->h_scratch.assign(cfg->max_seqs, 0);
 
     int dev = 0;
@@ -194,6 +196,7 @@ extern "C" int spork_seq_create(spork_ctx *c, int n, int32_t *ids_out) {
             c->h_live[s] = 1;
             c->h_len[s] = 0;
             c->h_shared_upto[s] = 0;
+            c->h_fork_key[s] = 0;
             ids_out[i++] = s;
         }
     c->n_live += n;

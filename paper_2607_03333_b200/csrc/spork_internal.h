@@ -115,6 +115,9 @@ struct spork_ctx {
     std::vector<int32_t> h_len;
     std::vector<uint8_t> h_live;
     std::vector<int32_t> h_shared_upto;  // pages below this index MAY be shared
+    std::vector<uint64_t> h_fork_key;    // (fork call, parent slot) the sequence was cloned by; 0: none / rolled back
+    std::vector<int32_t> h_fork_nf;      // full pages it shared with its parent at that fork
+    uint64_t fork_calls = 0;
     std::vector<int32_t> h_scratch;      // per-slot scratch (fork counts, evolving lens)
     int64_t free_lb;                     // lower bound on free pages
     int n_live;
