@@ -287,3 +287,41 @@ def test_parent_released_before_children():
     orc.release(ids[1:])
     spk.release(ids[1:])
     assert not spk.export_refcounts().any()
+
+
+# ---------------------------------------------------------------------------
+# fragmented pool (dummy sequences pin a random half of the pool)
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("path", ["auto", "mma.sync"])
+def test_fragmented_pool(path):
+    """Dummy sequences fill the pool, a random half of them is released, and the workload is built into
+    the holes: block tables are scattered page ids (lowest free id first, A-1), bit-exact on both
+    sides, and attention over them matches the oracle."""
+    cfg = synth.CFG5.scaled(n_groups=2, group_size=3, prefix_len=900, suffix_lo=1, suffix_hi=260)
+    wl = synth.Workload(cfg)
+    npg, ms, mp = pool_dims(wl, 64)
+    n_dummy = 120
+    orc = make_oracle(cfg, npg + n_dummy * 3, ms + n_dummy, mp)
+    spk = make_spork(cfg, npg + n_dummy * 3, ms + n_dummy, mp)
+    _set_path(spk, path)
+    r = np.random.default_rng(31)
+    dummies = orc.seq_create(n_dummy)
+    assert np.array_equal(dummies, spk.seq_create(n_dummy))
+    for s in dummies:                       # 1..3 pages each, interleaved
+        n = int(r.integers(1, 3 * 16 + 1))
+        k = synth.to_storage(r.standard_normal((n, cfg.Hkv, cfg.D), dtype=np.float32), cfg.dtype)
+        orc.append([s], [n], k, k)
+        spk.append([s], [n], k, k)
+    gone = r.permutation(dummies)[: n_dummy // 2]
+    orc.release(gone)
+    spk.release(gone)
+    ids = synth.build_state(orc, wl)
+    assert np.array_equal(ids, synth.build_state(spk, wl))
+    assert_state_equal(orc, spk, ids)
+    L, T = spk.export(int(ids[0]))
+    assert np.any(np.diff(T) != 1)          # really scattered
+    q = wl.q_all()
+    out_ref, lse_ref = orc.decode(ids, q)
+    out, lse = spk.decode_attn(wl.group_indptr(), ids, q)
+    check_attn(out, lse, out_ref, lse_ref, "bf16", "fragmented pool")
+    assert spk.last_plan()["n_prefix_items"] >= 1
