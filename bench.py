@@ -230,8 +230,8 @@ def run_ours(args, cfg, name, wl):
         spk.set_tensor_path_min_rows(args.min_rows)
     if args.stream_k is not None:
         spk.set_stream_k(bool(args.stream_k))
-    if args.two_pipe is not None:
-        spk.set_two_pipe(args.two_pipe)
+    if args.many_row_variant is not None:
+        spk.set_many_row_variant(args.many_row_variant)
     st = spk.stream
     gi = wl.group_indptr()
     qi = wl.q_indptr()
@@ -560,7 +560,7 @@ def main():
                     help="fork groups in the oracle's bounded sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stream-k", type=int, default=None, choices=[0, 1], help="planner knob: stream-K schedule")
-    ap.add_argument("--two-pipe", type=int, default=None, choices=[0, 1, 2],
+    ap.add_argument("--many-row-variant", type=int, default=None, choices=[0, 1, 2],
                     help="planner knob: > 128-row segments on the two-pipe tcgen05 kernel")
     ap.add_argument("--min-rows", type=int, default=None,
                     help="planner knob: rows per KV head from which a segment runs on the tcgen05 kernel")

@@ -274,7 +274,7 @@ int spork_set_tensor_path_min_rows(spork_ctx *ctx, int min_rows);
  * Results do not depend on the mode beyond rounding.  Other values are read as 0.  Invalidates
  * the cached plan.
  */
-int spork_set_two_pipe(spork_ctx *ctx, int mode);
+int spork_set_many_row_variant(spork_ctx *ctx, int mode);
 /*
  * Tuning knob: allow (default) or forbid the stream-K schedule.  Allowed: when every segment of
  * a call is a single row block of the tcgen05 kernel (every decode call on a bf16, D = 128

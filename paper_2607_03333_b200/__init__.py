@@ -32,7 +32,7 @@ ABI_SYMBOLS = [
     "spork_fork", "spork_release", "spork_truncate", "spork_decode_attn", "spork_verify_attn",
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
-    "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_two_pipe", "spork_set_stream_k", "spork_strerror",
+    "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_many_row_variant", "spork_set_stream_k", "spork_strerror",
 ]
 
 
@@ -94,7 +94,7 @@ def load(build_if_missing: bool = True):
         "spork_confidence": ([P, I, P, P, I, P, P], I),
         "spork_set_timing": ([P, I], I),
         "spork_set_tensor_path_min_rows": ([P, I], I),
-        "spork_set_two_pipe": ([P, I], I),
+        "spork_set_many_row_variant": ([P, I], I),
         "spork_set_stream_k": ([P, I], I),
         "spork_last_kernel_ms": ([P, P, P], I),
         "spork_strerror": ([I], C.c_char_p),
@@ -347,9 +347,9 @@ class Spork:
         """Planner knob: segments with >= min_rows rows per KV head run on the tcgen05 kernel."""
         self._chk(self.lib.spork_set_tensor_path_min_rows(self._h, int(min_rows)))
 
-    def set_two_pipe(self, enable: bool):
+    def set_many_row_variant(self, enable: bool):
         """Planner knob: run > 128-row segments on the two-pipe tcgen05 kernel (default on)."""
-        self._chk(self.lib.spork_set_two_pipe(self._h, int(enable)))
+        self._chk(self.lib.spork_set_many_row_variant(self._h, int(enable)))
 
     def set_stream_k(self, enable: bool):
         """Planner knob: equal-work contiguous schedule for single-row-block calls (default on)."""

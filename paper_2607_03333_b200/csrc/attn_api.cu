@@ -123,9 +123,9 @@ extern "C" int spork_set_tensor_path_min_rows(spork_ctx *c, int min_rows) {
     return SPORK_OK;
 }
 
-extern "C" int spork_set_two_pipe(spork_ctx *c, int enable) {
+extern "C" int spork_set_many_row_variant(spork_ctx *c, int enable) {
     if (!c) return SPORK_ERR_INVALID;
-    c->two_pipe = enable < 0 || enable > 2 ? 0 : enable;
+    c->many_row_variant = enable < 0 || enable > 2 ? 0 : enable;
     c->plan.valid = false;
     return SPORK_OK;
 }

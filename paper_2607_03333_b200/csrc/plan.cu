@@ -227,8 +227,8 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     int64_t total_cost = 0;
     for (Segment &s : segs) {
         const int rows = s.nq * G;
-        s.kind = !(mma && rows >= c->umma_min_rows) ? 0 : (rows > ROW_BLOCK_UMMA && c->two_pipe ? 2 : 1);
-        s.row_block = s.kind == 0 ? ROW_BLOCK : (s.kind == 2 && c->two_pipe == 1 ? 2 : 1) * ROW_BLOCK_UMMA;
+        s.kind = !(mma && rows >= c->umma_min_rows) ? 0 : (rows > ROW_BLOCK_UMMA && c->many_row_variant ? 2 : 1);
+        s.row_block = s.kind == 0 ? ROW_BLOCK : (s.kind == 2 && c->many_row_variant == 1 ? 2 : 1) * ROW_BLOCK_UMMA;
         int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);
         total_cost += (int64_t)tiles * Hkv * ceil_div(s.nq * G, s.row_block);
     }
@@ -238,7 +238,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     // once and read once by the merge kernel, which all CTAs share.  Fewer, longer items cost less
     // overhead and less partial traffic; more, shorter items balance the persistent CTAs better.
     const int grid_cap_umma = mma ? attn_umma_grid(c, 0) : 0;
-    const int grid_cap_umma2 = mma ? attn_umma_grid(c, c->two_pipe) : 0;
+    const int grid_cap_umma2 = mma ? attn_umma_grid(c, c->many_row_variant) : 0;
     auto split = [&](int chunk_tiles, int64_t *part_rows_out, size_t *n_items_out) -> bool {
         int64_t part_rows = 0;
         size_t n_items = 0;
@@ -266,7 +266,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
                 // a two-pipe CTA has the SM to itself: a tile takes it half the time of a one-pipe CTA
                 const float t = ((float)std::min(s.chunk_tiles, tiles - sp * s.chunk_tiles) +
                                  (kind ? ITEM_FIXED_COST_UMMA_CHUNKED : ITEM_FIXED_COST)) *
-                                (kind == 2 && c->two_pipe == 1 ? 0.5f : 1.f);
+                                (kind == 2 && c->many_row_variant == 1 ? 0.5f : 1.f);
                 cost.insert(cost.end(), (size_t)Hkv * n_rb, t);
             }
         }
@@ -493,7 +493,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     P.grid = grid;
     P.grid_umma = grid_umma;
     P.grid_umma2 = grid_umma2;
-    P.variant2 = c->two_pipe == 2 ? 2 : 1;
+    P.variant2 = c->many_row_variant == 2 ? 2 : 1;
     P.n_qrows = n_qrows;
     P.verify = verify;
     P.len_epoch = c->len_epoch;

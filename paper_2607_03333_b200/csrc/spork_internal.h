@@ -139,7 +139,7 @@ struct spork_ctx {
     bool plan_ev_pending;
     int timing = 0;
     int stream_k = 1;             // equal-work contiguous schedule when every segment is one row block
-    int two_pipe = 0;             // segments of > 128 rows: 0 default kernel, 1 two-pipe, 2 split-row kernel
+    int many_row_variant = 0;             // segments of > 128 rows: 0 default kernel, 1 two-pipe, 2 split-row kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;

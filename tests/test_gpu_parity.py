@@ -100,9 +100,9 @@ def _set_path(spk, path):
     if PATHS[path] is not None:
         spk.set_tensor_path_min_rows(PATHS[path])
     if path == "tcgen05-two-pipe":
-        spk.set_two_pipe(1)
+        spk.set_many_row_variant(1)
     if path == "tcgen05-split-row":
-        spk.set_two_pipe(2)
+        spk.set_many_row_variant(2)
 
 
 def _check_kernel(info, path):
