@@ -188,6 +188,16 @@ def run_reference(args, cfg, name, wl):
     print(json.dumps(line))
 
 
+def _traffic(workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the workload's dominant kernel, from
+    the committed ncu capture (profiles/traffic.json); None if there is none."""
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            return json.load(f).get(workload)
+    return None
+
+
 def max_over_ranks(x: float, device, world: int) -> float:
     """Replicas only: the step time of an N-replica run is the slowest rank's."""
     if world <= 1:
@@ -319,11 +329,7 @@ def run_ours(args, cfg, name, wl):
         peak_tf = float(peaks["bf16_tflops"])
         ach_tf = flops / (k_avg * 1e-3) / 1e12
         tensor_bound = verify and (flops / (peak_tf * 1e12)) > (ub / (peak_bw * 1e9))
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tpath):
-            with open(tpath) as f:
-                traffic = json.load(f).get(name)
+        traffic = _traffic(name)
         if tensor_bound:
             roof = {"bound": "tensor", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / peak_tf, "traffic": traffic}
@@ -538,7 +544,7 @@ def run_d2(args):
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "clocks": clocks, "gpu_launches": 2 * args.steps,
             "roofline": {"bound": "hbm", "achieved": ach, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
-                         "frac": ach / float(peaks["hbm_gbs"]), "traffic": None,
+                         "frac": ach / float(peaks["hbm_gbs"]), "traffic": _traffic(name),
                          "kernel": "conf_partial_kernel+conf_span_kernel (whole call)",
                          "peak_source": peaks["_source"], "algorithmic_bytes": alg_bytes},
             "e2e": {"value": aggregate_value(alg_bytes, e_ms, world), "unit": "GB/s", "ms_per_step": e_ms,
