@@ -1,15 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line per run (the driver's contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2|3|4|5|churn|d2] [--k 4|8|16]
-                    [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|churn|loop|layers|d2]
+                    [--k 4|8|16] [--impl reference]
 
 A step = one pass of the hot path over one batch of synthetic input:
   configs 2/3/5  one spork_decode_attn call (plan lookup, cascade decode kernel, merge kernel)
   config 4       one spork_verify_attn call with k drafts per sequence
-  churn          one spork_fork of 10,000 children + one spork_release of them (config 5)
+  config 1       the tiny fp32 group (us/step only: launch-latency bound, no roofline target)
+  churn          one spork_fork of 10,000 children + one spork_release of them (config 5, 2^20-page pool)
+  loop           spork_append of one token to every sequence + spork_decode_attn (Alg. 1 step 5,
+                 PAPER.md:261; the paper's decode loop), on config 2
   d2             one spork_confidence call: Eq. 2 over 256 probe spans of Qwen3-vocabulary logits
-Default workload: BASELINE.json configs[1] (Qwen3-4B shape, 16 fork groups of 2, prefix 4096).
+Default (`--config all`): the headline is the LARGEST single-GPU decode config of BASELINE.json
+(config 5: 16 fork groups of 8, prefix 32768, 1.59 GB of unique KV); the same JSON line carries a
+`per_config` object with the same measurements for config 2, config 3, config 4 at k = 4, 8, 16
+(with verify TFLOP/s), the fork churn, the append+decode loop and config 1.
 Inputs are seeded synthetic (synth/), resident in HBM before the timed region; L2 is flushed
 between timed iterations.  `value` = unique KV bytes / step time (GB/s); config 4 also reports
 TFLOP/s.  N > 1 (torchrun) runs N independent replicas: the path does not shard ("replicas only").
@@ -17,6 +23,7 @@ TFLOP/s.  N > 1 (torchrun) runs N independent replicas: the path does not shard 
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import subprocess
@@ -34,6 +41,9 @@ import synth  # noqa: E402
 
 METRIC = "forked_decode_attn_unique_kv_bandwidth"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+L2_NOTE = "flushed between timed iterations (512 MiB write, then 256 MiB read so no dirty lines remain)"
+OUT_TOL = {"f32": 1e-5, "bf16": 1e-2}     # BASELINE.json north_star
+LSE_RTOL = 1e-4
 
 
 def load_peaks():
@@ -71,6 +81,7 @@ class ClockSampler:
             self.t.start()
         except Exception:
             self.proc = None
+        return self
 
     def _read(self):
         for line in self.proc.stdout:
@@ -107,15 +118,10 @@ class ClockSampler:
 # ---------------------------------------------------------------------------
 # workloads
 # ---------------------------------------------------------------------------
-def pick_config(args):
-    if args.config == "churn":
-        return synth.CFG5, "cfg5_fork_churn"
-    n = int(args.config)
-    cfg = synth.CONFIGS[n]
-    if n == 4:
-        cfg = cfg.scaled(k_draft=args.k)
-        return cfg, f"cfg4_qwen3_32b_verify_k{args.k}"
-    return cfg, cfg.name
+def workload_name(cfg) -> str:
+    if cfg.cfg_no == 4:
+        return f"cfg4_qwen3_32b_verify_k{cfg.k_draft}"
+    return cfg.name
 
 
 def pool_dims(wl, num_pages=None):
@@ -125,24 +131,27 @@ def pool_dims(wl, num_pages=None):
     return (num_pages or need + 1024), per_seq
 
 
-def build_spork(cfg, wl, num_pages=None, max_seqs=None, device="cuda:0"):
+def build_spork(cfg, wl, num_pages=None, max_seqs=None, device="cuda:0", extra_pages_per_seq=0):
     import paper_2607_03333_b200 as sp
     npg, mp = pool_dims(wl, num_pages)
-    spk = sp.Spork(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, npg, max_seqs or cfg.n_seqs + 8, mp, cfg.scale,
-                   device=device)
+    spk = sp.Spork(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, npg, max_seqs or cfg.n_seqs + 8, mp + extra_pages_per_seq,
+                   cfg.scale, device=device)
     ids = synth.build_state(spk, wl)
     spk.synchronize()
     return spk, ids
 
 
 # ---------------------------------------------------------------------------
-# the oracle leg (cpu_baseline and --impl reference): a bounded sample of the same workload
+# the oracle leg (cpu_baseline, parity spot check, --impl reference): bounded samples of the workload
 # ---------------------------------------------------------------------------
-def oracle_sample(cfg, wl, max_groups=2):
+REF_GROUPS = {1: 1, 2: 16, 3: 8, 4: 2, 5: 4}
+
+
+def oracle_sample(cfg, wl, max_groups=0):
     """Builds `max_groups` fork groups of the workload in the CPU oracle and returns a closure that
     runs one oracle step on them, plus the factor that scales its time to the whole batch."""
     import oracle
-    g = min(cfg.n_groups, max_groups)
+    g = min(cfg.n_groups, max_groups or REF_GROUPS[cfg.cfg_no])
     sub = cfg.scaled(n_groups=g)
     # same sub-streams as the full workload: groups / sequences [0, g) are identical
     swl = synth.Workload(sub, wl.k[:sub.n_seqs] if cfg.k_draft else None)
@@ -164,7 +173,50 @@ def oracle_sample(cfg, wl, max_groups=2):
     return step, frac, oracle.num_threads(), f"{g} of {cfg.n_groups} fork groups ({sub.n_seqs} sequences), all heads"
 
 
-def run_reference(args, cfg, name, wl):
+def cpu_baseline_attn(cfg, wl, ub, max_groups=0):
+    ostep, frac, cores, sample = oracle_sample(cfg, wl, max_groups)
+    # repeat the sample until about a second of wall clock (>= 10 core-seconds on this box's host
+    # cores) has been spent; the mean step of the sample is scaled to the whole batch by flops
+    reps, t0 = 0, time.perf_counter()
+    while reps < 20 and (reps == 0 or time.perf_counter() - t0 < 1.0):
+        ostep()
+        reps += 1
+    dt = (time.perf_counter() - t0) / reps
+    return {"value": ub / (dt / frac) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+            "sample": sample + f", {reps} repetition(s)", "sample_seconds": dt * reps,
+            "scaled_ms_per_step": dt / frac * 1e3}
+
+
+def parity_spot_check(cfg, wl, out_np, lse_np, n_rows=2, seed=0):
+    """What was just timed, against the oracle's plain dense definition on regenerated K/V: `n_rows`
+    sampled (sequence, draft row) pairs, ALL heads of each.  Asserts the north_star tolerances."""
+    import oracle
+    r = np.random.default_rng([23, cfg.cfg_no, seed])
+    qi = wl.q_indptr()
+    worst, worst_l = 0.0, 0.0
+    for _ in range(n_rows):
+        seq = int(r.integers(0, cfg.n_seqs))
+        k = int(wl.k[seq])
+        j = int(r.integers(0, max(1, k)))
+        K, V = wl.dense_kv(seq)
+        Q = wl.q(seq)
+        L = int(wl.total_len[seq])
+        n_att = L if k == 0 else L - k + j + 1
+        row = int(qi[seq]) + j
+        for h in range(cfg.Hq):
+            o_ref, l_ref = oracle.attend_dense(cfg.dtype, cfg.scale, Q[j, h], K[:n_att, h // cfg.G],
+                                               V[:n_att, h // cfg.G])
+            err = float(np.max(np.abs(out_np[row, h].astype(np.float64) - o_ref)))
+            lerr = abs(float(lse_np[row, h]) - l_ref) / max(1.0, abs(l_ref))
+            worst, worst_l = max(worst, err), max(worst_l, lerr)
+    assert worst <= OUT_TOL[cfg.dtype] and worst_l <= LSE_RTOL, \
+        f"bench output does not match the oracle: out err {worst:.3e}, lse rel err {worst_l:.3e}"
+    return {"rows_checked": n_rows * cfg.Hq, "max_abs_err": worst, "max_lse_rel_err": worst_l,
+            "tolerance": OUT_TOL[cfg.dtype], "against": "oracle.attend_dense (fp64)"}
+
+
+def reference_line(args, cfg, wl):
+    name = workload_name(cfg)
     step, frac, cores, sample = oracle_sample(cfg, wl, args.ref_groups)
     for _ in range(max(0, min(args.warmup, 1))):
         step()
@@ -176,7 +228,7 @@ def run_reference(args, cfg, name, wl):
     full = dt / frac                       # time one whole step would take, scaled by flops
     ub = wl.unique_kv_bytes()
     val = ub / full / 1e9
-    line = {
+    return {
         "impl": "reference", "metric": METRIC, "value": val, "unit": "GB/s", "n_gpus": args.gpus,
         "steps": steps, "warmup": args.warmup, "ms_per_step": full * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
@@ -185,7 +237,6 @@ def run_reference(args, cfg, name, wl):
         "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
-    print(json.dumps(line))
 
 
 def _traffic(workload: str):
@@ -217,218 +268,480 @@ def aggregate_value(unique_bytes: int, ms_step: float, world: int) -> float:
 # ---------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------
-def run_ours(args, cfg, name, wl):
-    import torch
-    import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
-    device = f"cuda:{local}"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(device))
-    peaks = load_peaks()
+class Env:
+    """Per-process GPU context shared by all records of a run."""
 
-    churn = args.config == "churn"
-    num_pages = (1 << 20) if (churn or (args.config == "5" and args.full_pool)) else None
-    max_seqs = cfg.n_seqs + 10008 if churn else None
-    t_build = time.perf_counter()
-    spk, ids = build_spork(cfg, wl, num_pages, max_seqs, device)
-    t_build = time.perf_counter() - t_build
-    if args.min_rows is not None:
-        spk.set_tensor_path_min_rows(args.min_rows)
-    if args.stream_k is not None:
-        spk.set_stream_k(bool(args.stream_k))
-    if args.many_row_variant is not None:
-        spk.set_many_row_variant(args.many_row_variant)
-    st = spk.stream
-    gi = wl.group_indptr()
-    qi = wl.q_indptr()
-    verify = cfg.k_draft > 0
-    q_np = wl.q_all()
-    q_dev = spk._dev(q_np)
-    rows = q_np.shape[0]
-    out = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32, device=device)
-    lse = torch.empty((rows, cfg.Hq), dtype=torch.float32, device=device)
-    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
-    clean = torch.zeros(64 << 20, dtype=torch.int32, device=device)    # 256 MiB, only ever read
-    parents = synth.churn_parents(5, 10000, ids) if churn else None
+    def __init__(self, args):
+        import torch
+        self.torch = torch
+        self.args = args
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+        self.device = f"cuda:{self.local}"
+        torch.cuda.set_device(self.local)
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("nccl", device_id=torch.device(self.device))
+        self.peaks = load_peaks()
+        self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=self.device)   # > 126 MB L2
+        self.clean = torch.zeros(64 << 20, dtype=torch.int32, device=self.device)    # 256 MiB, only ever read
 
-    churn_launches = [0]
-
-    def step():
-        if churn:
-            ch = spk.fork(parents)
-            n1 = spk.last_launches()
-            spk.release(ch)
-            churn_launches[0] = n1 + spk.last_launches()
-        elif verify:
-            spk.verify_attn(gi, ids, qi, q_dev, out, lse)
-        else:
-            spk.decode_attn(gi, ids, q_dev, out, lse)
-
-    def flush_l2():
+    def flush_l2(self, st):
         # write 512 MiB (evicts every line of the workload), then read 256 MiB of unrelated data so
         # the dirty lines are written back BEFORE the timed region: L2 starts cold and clean
-        with torch.cuda.stream(st):
-            flush.zero_()
-            clean.max()
+        with self.torch.cuda.stream(st):
+            self.flush.zero_()
+            self.clean.max()
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
+    def barrier(self):
+        self.torch.cuda.synchronize()
+        if self.world > 1:
+            import torch.distributed as dist
             dist.barrier()
-        torch.cuda.synchronize()
+        self.torch.cuda.synchronize()
 
-    def timed(n, do_flush=True):
+    def timed(self, st, step, n, do_flush=True, pre=None):
+        """CUDA events on the launch stream around each of n steps (L2 flushed before each)."""
+        torch = self.torch
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(n)]
         for a, b in evs:
+            if pre is not None:
+                pre()
             if do_flush:
-                flush_l2()
+                self.flush_l2(st)
             a.record(st)
             step()
             b.record(st)
         torch.cuda.synchronize()
         return [a.elapsed_time(b) for a, b in evs]
 
+    def mx(self, x):
+        return max_over_ranks(float(x), self.device, self.world)
+
+    def close(self):
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.destroy_process_group()
+
+
+def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
+    """One record: step time, roofline of the dominant kernel, e2e through the host-buffer ABI calls,
+    the oracle on the host cores, and a parity spot check of the timed output."""
+    torch, args = env.torch, env.args
+    name = workload_name(cfg)
+    st = spk.stream
+    gi, qi = wl.group_indptr(), wl.q_indptr()
+    verify = cfg.k_draft > 0
+    q_np = wl.q_all()
+    q_dev = spk._dev(q_np)
+    rows = q_np.shape[0]
+    out = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32, device=env.device)
+    lse = torch.empty((rows, cfg.Hq), dtype=torch.float32, device=env.device)
+
+    def step():
+        if verify:
+            spk.verify_attn(gi, ids, qi, q_dev, out, lse)
+        else:
+            spk.decode_attn(gi, ids, q_dev, out, lse)
+
     # nvidia-smi samples every 100 ms: the sampler runs from the warm-up to the end of the e2e pass
     # (the GPU is under the same load throughout), the timed region lies inside that window
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler = ClockSampler(env.local).start()
+    t0 = time.perf_counter()
+    step()
+    spk.synchronize()
+    first_call_us = (time.perf_counter() - t0) * 1e6      # plan build + upload + first launch, host clock
+    info0 = spk.last_plan()
     for _ in range(max(args.warmup, 3)):
-        flush_l2()
+        env.flush_l2(st)
         step()
-    barrier()
-    ms = timed(args.steps)
-    barrier()
-    total_ms = max_over_ranks(float(sum(ms)), device, world)
-    ms_step = total_ms / args.steps
-
-    info = spk.last_plan() if not churn else {}
-    ub = wl.unique_kv_bytes() if not churn else 0
+    env.barrier()
+    ms = env.timed(st, step, args.steps)
+    env.barrier()
+    ms_step = env.mx(sum(ms)) / args.steps
+    info = spk.last_plan()
+    ub = wl.unique_kv_bytes()
+    assert info["unique_tokens"] * cfg.token_bytes == ub, "library and synth disagree on the unique KV bytes"
     flops = wl.flops()
-    launches_per_step = info.get("launches", 0) if not churn else churn_launches[0]
 
     # ---- roofline of the dominant kernel (separate timed pass with kernel events on) ----
-    roof = None
-    extra = {}
-    if not churn:
-        spk.set_timing(True)
-        k_ms, m_ms = [], []
-        for _ in range(args.steps):
-            flush_l2()
-            step()
-            a, m = spk.last_kernel_ms()
-            k_ms.append(a)
-            m_ms.append(m)
-        spk.set_timing(False)
-        k_avg = float(np.mean(k_ms))
-        peak_bw = float(peaks["hbm_gbs"])
-        ach_bw = info["unique_tokens"] * cfg.token_bytes / (k_avg * 1e-3) / 1e9
-        peak_tf = float(peaks["bf16_tflops"])
-        ach_tf = flops / (k_avg * 1e-3) / 1e12
-        tensor_bound = verify and (flops / (peak_tf * 1e12)) > (ub / (peak_bw * 1e9))
-        traffic = _traffic(name)
-        if tensor_bound:
-            roof = {"bound": "tensor", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                    "frac": ach_tf / peak_tf, "traffic": traffic}
-        else:
-            roof = {"bound": "hbm", "achieved": ach_bw, "peak": peak_bw, "unit": "GB/s",
-                    "frac": ach_bw / peak_bw, "traffic": traffic}
-        kname = {0: "attn_simt_kernel", 1: "attn_mma_kernel", 2: "attn_umma_kernel",
-                 3: "attn_umma_kernel+attn_mma_kernel"}[info["kernel"]]
-        roof.update({"kernel": kname,
-                     "kernel_ms": k_avg, "merge_ms": float(np.mean(m_ms)), "peak_source": peaks["_source"],
-                     "frac_of_8TBps": ach_bw / 8000.0, "achieved_tflops": ach_tf,
-                     "algorithmic_bytes": info["unique_tokens"] * cfg.token_bytes})
-        warm = timed(args.steps, do_flush=False)
-        extra["warm_l2_ms_per_step"] = float(np.mean(warm))
-        extra["plan"] = info
+    peaks = env.peaks
+    spk.set_timing(True)
+    k_ms, m_ms = [], []
+    for _ in range(args.steps):
+        env.flush_l2(st)
+        step()
+        a, m = spk.last_kernel_ms()
+        k_ms.append(a)
+        m_ms.append(m)
+    spk.set_timing(False)
+    k_avg = float(np.mean(k_ms))
+    bf16_path = info["kernel"] != 0
+    peak_bw, peak_tf = float(peaks["hbm_gbs"]), float(peaks["bf16_tflops"])
+    ach_bw = ub / (k_avg * 1e-3) / 1e9
+    ach_tf = flops / (k_avg * 1e-3) / 1e12
+    tensor_bound = verify and bf16_path and (flops / (peak_tf * 1e12)) > (ub / (peak_bw * 1e9))
+    kname = {0: "attn_simt_kernel", 1: "attn_mma_kernel", 2: "attn_umma_kernel",
+             3: "attn_umma_kernel+attn_mma_kernel"}[info["kernel"]]
+    if tensor_bound:
+        roof = {"bound": "tensor", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach_tf / peak_tf, "traffic": _traffic(name)}
+    else:
+        roof = {"bound": "hbm", "achieved": ach_bw, "peak": peak_bw, "unit": "GB/s",
+                "frac": ach_bw / peak_bw, "traffic": _traffic(name)}
+    roof.update({"kernel": kname, "kernel_ms": k_avg, "merge_ms": float(np.mean(m_ms)),
+                 "peak_source": peaks["_source"], "frac_of_8TBps": ach_bw / 8000.0,
+                 "achieved_tflops": ach_tf, "algorithmic_bytes": ub, "algorithmic_flops": flops})
+    warm = env.timed(st, step, args.steps, do_flush=False)
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region ----
-    e2e = None
-    if not churn:
-        qh = torch.from_numpy(q_np).pin_memory()
-        oh = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32).pin_memory()
-        lh = torch.empty((rows, cfg.Hq), dtype=torch.float32).pin_memory()
+    qh = torch.from_numpy(q_np).pin_memory()
+    oh = torch.empty((rows, cfg.Hq, cfg.D), dtype=torch.float32).pin_memory()
+    lh = torch.empty((rows, cfg.Hq), dtype=torch.float32).pin_memory()
 
-        def e2e_step():
-            if verify:
-                spk.verify_attn_host(gi, ids, qi, qh, oh, lh)
-            else:
-                spk.decode_attn_host(gi, ids, qh, oh, lh)
+    def e2e_step():
+        if verify:
+            spk.verify_attn_host(gi, ids, qi, qh, oh, lh)
+        else:
+            spk.decode_attn_host(gi, ids, qh, oh, lh)
 
-        for _ in range(3):
-            e2e_step()
-        tt = []
-        for _ in range(args.steps):
-            flush_l2()
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            e2e_step()
-            tt.append(time.perf_counter() - t0)
-        e_ms = max_over_ranks(float(np.mean(tt)) * 1e3, device, world)
-        e2e = {"value": aggregate_value(ub, e_ms, world), "unit": "GB/s", "ms_per_step": e_ms,
-               "h2d_bytes_per_step": int(qh.numel() * qh.element_size()),
-               "d2h_bytes_per_step": int(oh.numel() * 4 + lh.numel() * 4)}
-        # parity spot check of what was just timed (oracle, one sampled row)
-        o = oh.numpy()
-        assert np.all(np.isfinite(o))
-
+    for _ in range(3):
+        e2e_step()
+    tt = []
+    for _ in range(args.steps):
+        env.flush_l2(st)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e2e_step()
+        tt.append(time.perf_counter() - t0)
+    e_ms = env.mx(float(np.mean(tt)) * 1e3)
+    e2e = {"value": aggregate_value(ub, e_ms, env.world), "unit": "GB/s", "ms_per_step": e_ms,
+           "h2d_bytes_per_step": int(qh.numel() * qh.element_size()),
+           "d2h_bytes_per_step": int(oh.numel() * 4 + lh.numel() * 4)}
     clocks = sampler.stop()
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
 
-    cpu = None
-    if not args.no_cpu_baseline and not churn:
-        ostep, frac, cores, sample = oracle_sample(cfg, wl, args.ref_groups)
-        # repeat the sample until about a second of wall clock (>= 10 core-seconds on this box's
-        # host cores) has been spent; the mean step of the sample is scaled to the whole batch by flops
-        reps, t0 = 0, time.perf_counter()
-        while reps < 20 and (reps == 0 or time.perf_counter() - t0 < 1.0):
-            ostep()
-            reps += 1
-        dt = (time.perf_counter() - t0) / reps
-        cpu = {"value": ub / (dt / frac) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
-               "sample": sample + f", {reps} repetition(s)", "sample_seconds": dt * reps,
-               "scaled_ms_per_step": dt / frac * 1e3}
-
-    if churn:
-        value, unit, metric = 10000 / (ms_step * 1e-3), "forks/s", "fork_release_churn"
-    else:
-        value, unit, metric = aggregate_value(ub, ms_step, world), "GB/s", METRIC
-    line = {
-        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype,
-        "data": "synthetic",
-        "config": {"workload": name, "Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_groups": cfg.n_groups,
-                   "group_size": cfg.group_size, "prefix_len": cfg.prefix_len,
-                   "suffix": [cfg.suffix_lo, cfg.suffix_hi], "k_draft": cfg.k_draft,
-                   "unique_kv_bytes": ub, "naive_kv_bytes": wl.naive_tokens() * cfg.token_bytes,
-                   "flops": flops, "l2": "flushed between timed iterations (512 MiB write, then 256 MiB read so no dirty lines remain)",
-                   "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "state_build_seconds": t_build},
-        "clocks": clocks,
-        "gpu_launches": int(launches_per_step * args.steps),
-        "frac_of_8TBps": (value / world / 8000.0) if not churn else None,
-        "frac_of_measured_hbm": (value / world / float(peaks["hbm_gbs"])) if not churn else None,
+    rec = {
+        "workload": name, "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
+        "value": aggregate_value(ub, ms_step, env.world), "unit": "GB/s",
+        "frac_of_8TBps": ub / (ms_step * 1e-3) / 1e9 / 8000.0,
+        "frac_of_measured_hbm": ub / (ms_step * 1e-3) / 1e9 / peak_bw,
+        "dtype": cfg.dtype, "unique_kv_bytes": ub, "naive_kv_bytes": wl.naive_tokens() * cfg.token_bytes,
+        "flops": flops, "roofline": roof, "e2e": e2e, "clocks": clocks,
+        "warm_l2_ms_per_step": float(np.mean(warm)), "first_call_us": first_call_us,
+        "plan_rebuild_us": info0.get("plan_host_us"), "launches_per_step": info["launches"], "plan": info,
+        "shape": {"Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_groups": cfg.n_groups,
+                  "group_size": cfg.group_size, "prefix_len": cfg.prefix_len,
+                  "suffix": [cfg.suffix_lo, cfg.suffix_hi], "k_draft": cfg.k_draft},
     }
     if verify:
-        line["verify_tflops"] = flops / (ms_step * 1e-3) / 1e12
-    if roof is not None:
-        line["roofline"] = roof
-    if e2e is not None:
-        line["e2e"] = e2e
-    if cpu is not None:
-        line["cpu_baseline"] = cpu
-    line.update(extra)
-    print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+        rec["verify_tflops"] = flops / (ms_step * 1e-3) / 1e12
+    if env.rank == 0 and cpu and not args.no_cpu_baseline:
+        rec["parity"] = parity_spot_check(cfg, wl, oh.numpy(), lh.numpy())
+        rec["cpu_baseline"] = cpu_baseline_attn(cfg, wl, ub, args.ref_groups)
+    return rec
+
+
+def churn_bytes(cfg, wl, ids, parents, num_pages):
+    """Algorithmic bytes of the churn step (SURVEY.md 8(d) churn row, computed exactly): fork = the
+    children's table rows read + written (floor(L/16) + 1 entries of 4 B), the duplicated tail pages
+    read + written (K and V), one scan of the refcount array; release = the children's table rows
+    read once more."""
+    L = {int(s): int(wl.total_len[i]) for i, s in enumerate(ids)}
+    page_bytes = cfg.Hkv * 16 * cfg.D * cfg.elt_bytes          # one pool
+    entries = sum(L[int(p)] // 16 + 1 for p in parents)
+    tails = sum(1 for p in parents if L[int(p)] % 16)
+    fork_clone = 2 * 4 * entries + tails * 2 * 2 * page_bytes
+    return {"fork_clone_kernel": fork_clone, "refcount_scan": 4 * num_pages, "release_table_read": 4 * entries,
+            "step": fork_clone + 4 * num_pages + 4 * entries, "table_entries": entries, "tail_pages": tails}
+
+
+def measure_churn(env: Env, spk, ids, cfg, wl, num_pages):
+    """config 5 fork stress: 10,000 spork_fork + spork_release per step on the 2^20-page pool."""
+    args = env.args
+    st = spk.stream
+    parents = synth.churn_parents(5, 10000, ids)
+    launches = [0]
+
+    def step():
+        ch = spk.fork(parents)
+        n1 = spk.last_launches()
+        spk.release(ch)
+        launches[0] = n1 + spk.last_launches()
+
+    sampler = ClockSampler(env.local).start()
+    for _ in range(max(args.warmup, 3)):
+        env.flush_l2(st)
+        step()
+    env.barrier()
+    ms = env.timed(st, step, args.steps)
+    env.barrier()
+    ms_step = env.mx(sum(ms)) / args.steps
+    # dominant kernel: fork_clone_kernel (table rows + tail pages), timed live with events on the stream
+    spk.set_timing(True)
+    k_ms = []
+    for _ in range(args.steps):
+        env.flush_l2(st)
+        ch = spk.fork(parents)
+        k_ms.append(spk.last_kernel_ms()[0])
+        spk.release(ch)
+    spk.set_timing(False)
+    clocks = sampler.stop()
+    k_avg = float(np.mean(k_ms))
+    by = churn_bytes(cfg, wl, ids, parents, num_pages)
+    peak_bw = float(env.peaks["hbm_gbs"])
+    ach = by["fork_clone_kernel"] / (k_avg * 1e-3) / 1e9
+    rec = {
+        "workload": "cfg5_fork_churn", "ms_per_step": ms_step, "us_per_step": ms_step * 1e3,
+        "value": env.world * 10000 / (ms_step * 1e-3), "unit": "forks/s", "dtype": "int32",
+        "step_gbs": by["step"] / (ms_step * 1e-3) / 1e9, "algorithmic_bytes_step": by["step"],
+        "roofline": {"bound": "hbm", "achieved": ach, "peak": peak_bw, "unit": "GB/s", "frac": ach / peak_bw,
+                     "traffic": _traffic("cfg5_fork_churn"), "kernel": "fork_clone_kernel", "kernel_ms": k_avg,
+                     "peak_source": env.peaks["_source"], "algorithmic_bytes": by["fork_clone_kernel"]},
+        "e2e": {"value": env.world * 10000 / (ms_step * 1e-3), "unit": "forks/s", "ms_per_step": ms_step,
+                "h2d_bytes_per_step": 4 * 10000 * 2, "d2h_bytes_per_step": 0,
+                "note": "the ABI takes HOST id arrays: the timed step already contains their staging copies"},
+        "clocks": clocks, "launches_per_step": launches[0], "bytes": by,
+        "shape": {"forks": 10000, "live_parents": int(len(ids)), "num_pages": num_pages},
+    }
+    if env.rank == 0 and not args.no_cpu_baseline:
+        rec["cpu_baseline"] = cpu_baseline_churn(cfg, wl, num_pages)
+    return rec
+
+
+def cpu_baseline_churn(cfg, wl, num_pages, n_forks=10000):
+    """oracle fork x 10,000 + release on the 2^20-page pool, single thread (the
+    lowest-free-id policy is sequential).  State is built with lengths only (no KV values: the oracle's
+    allocator does not look at them; its tail copies are skipped)."""
+    import oracle
+    npg, mp = pool_dims(wl, num_pages)
+    orc = oracle.Oracle(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, npg, cfg.n_seqs + n_forks + 8, mp, cfg.scale,
+                        store_kv=False)
+    ids = synth.build_state(orc, wl, values=False)
+    parents = synth.churn_parents(5, n_forks, ids)
+    t0 = time.perf_counter()
+    ch = orc.fork(parents)
+    orc.release(ch)
+    dt = time.perf_counter() - t0
+    return {"value": n_forks / dt, "unit": "forks/s", "cores": 1, "kind": "oracle",
+            "sample": f"the whole step once: {n_forks} forks + releases, table and refcount work only (no tail copies)",
+            "sample_seconds": dt, "scaled_ms_per_step": dt * 1e3}
+
+
+def measure_cfg1(env: Env):
+    """config 1: us/step of the tiny fp32 fork group (launch latency; excluded from the 70 % target)."""
+    args = env.args
+    cfg = synth.CFG1
+    wl = synth.Workload(cfg)
+    spk, ids = build_spork(cfg, wl, device=env.device)
+    st = spk.stream
+    gi = wl.group_indptr()
+    q_np = wl.q_all()
+    q_dev = spk._dev(q_np)
+    out, lse = spk.decode_attn(gi, ids, q_dev)
+
+    def step():
+        spk.decode_attn(gi, ids, q_dev, out, lse)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    ms = env.timed(st, step, args.steps)
+    ms_step = env.mx(sum(ms)) / args.steps
+    spk.set_timing(True)
+    k_ms = []
+    for _ in range(args.steps):
+        step()
+        k_ms.append(spk.last_kernel_ms()[0])
+    spk.set_timing(False)
+    ub = wl.unique_kv_bytes()
+    rec = {"workload": cfg.name, "ms_per_step": ms_step, "us_per_step": ms_step * 1e3, "dtype": "f32",
+           "value": aggregate_value(ub, ms_step, env.world), "unit": "GB/s", "unique_kv_bytes": ub,
+           "roofline": None, "kernel": "attn_simt_kernel", "kernel_ms": float(np.mean(k_ms)),
+           "note": "0.16 MB problem: launch-latency bound, excluded from the 70 % target (SURVEY 8(d))",
+           "plan": spk.last_plan()}
+    if env.rank == 0 and not args.no_cpu_baseline:
+        import oracle
+        o = oracle.Oracle(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, 64, 8, 32, cfg.scale)
+        oids = synth.build_state(o, wl)
+        ref, lref = o.decode(oids, q_np)
+        err = float(np.max(np.abs(out.cpu().numpy() - ref)))
+        assert err <= OUT_TOL["f32"], f"config 1 does not match the oracle: {err:.3e}"
+        t0 = time.perf_counter()
+        for _ in range(20):
+            o.decode(oids, q_np)
+        dt = (time.perf_counter() - t0) / 20
+        rec["parity"] = {"rows_checked": int(ref.shape[0] * ref.shape[1]), "max_abs_err": err, "tolerance": 1e-5}
+        rec["cpu_baseline"] = {"value": ub / dt / 1e9, "unit": "GB/s", "cores": oracle.num_threads(),
+                               "kind": "oracle", "sample": "the whole step, 20 repetitions",
+                               "scaled_ms_per_step": dt * 1e3}
+    spk.close()
+    return rec
+
+
+def measure_loop(env: Env, cfg, n_steps=None):
+    """The paper's decode loop (Alg. 1 step 5; SURVEY 8(b) call order): each timed step
+    appends ONE token to every sequence and then attends.  Reports the step, the append's share and
+    how often the plan had to be rebuilt."""
+    torch, args = env.torch, env.args
+    wl = synth.Workload(cfg)
+    n_steps = n_steps or max(args.steps, 64)
+    total = n_steps + max(args.warmup, 3) + 8
+    spk, ids = build_spork(cfg, wl, device=env.device, extra_pages_per_seq=total // 16 + 2,
+                           num_pages=pool_dims(wl)[0] + cfg.n_seqs * (total // 16 + 2))
+    st = spk.stream
+    gi = wl.group_indptr()
+    q_dev = spk._dev(wl.q_all())
+    out = torch.empty((cfg.n_seqs, cfg.Hq, cfg.D), dtype=torch.float32, device=env.device)
+    lse = torch.empty((cfg.n_seqs, cfg.Hq), dtype=torch.float32, device=env.device)
+    r = synth.rng(cfg.cfg_no, synth.T_MISC, 77)
+    kv = spk._dev(synth.to_storage(r.standard_normal((2, cfg.n_seqs, cfg.Hkv, cfg.D), dtype=np.float32), cfg.dtype))
+    ones = np.ones(cfg.n_seqs, np.int32)
+    cached, rebuild_us = [], []
+
+    def step():
+        spk.append(ids, ones, kv[0], kv[1])
+        spk.decode_attn(gi, ids, q_dev, out, lse)
+
+    for _ in range(max(args.warmup, 3)):
+        env.flush_l2(st)
+        step()
+    env.barrier()
+    evs = []
+    for _ in range(n_steps):
+        env.flush_l2(st)
+        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        a.record(st)
+        spk.append(ids, ones, kv[0], kv[1])
+        b.record(st)
+        spk.decode_attn(gi, ids, q_dev, out, lse)
+        c.record(st)
+        info = spk.last_plan()
+        cached.append(info["plan_cached"])
+        if not info["plan_cached"]:
+            rebuild_us.append(info.get("plan_host_us"))
+        evs.append((a, b, c))
+    torch.cuda.synchronize()
+    env.barrier()
+    app = float(np.mean([a.elapsed_time(b) for a, b, _ in evs]))
+    att = float(np.mean([b.elapsed_time(c) for _, b, c in evs]))
+    ms_step = env.mx(float(np.mean([a.elapsed_time(c) for a, _, c in evs])))
+    # host-side pace: the same loop without flushes or events, wall clock per step
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        step()
+    torch.cuda.synchronize()
+    wall = (time.perf_counter() - t0) / n_steps
+    L_end = wl.total_len + (2 * n_steps + 2 * max(args.warmup, 3))
+    spk.close()
+    return {"workload": f"{cfg.name}_append_decode_loop", "steps": n_steps, "ms_per_step": ms_step,
+            "us_per_step": ms_step * 1e3, "append_us": app * 1e3, "attn_us": att * 1e3,
+            "wall_us_per_step_back_to_back": wall * 1e6,
+            "plan_cached_frac": float(np.mean(cached)), "plan_rebuilds": int(len(cached) - sum(cached)),
+            "plan_rebuild_us": float(np.mean([x for x in rebuild_us if x is not None])) if any(
+                x is not None for x in rebuild_us) else None,
+            "value": aggregate_value(wl.unique_kv_bytes(), ms_step, env.world), "unit": "GB/s",
+            "note": "unique KV bytes of the initial state; sequences grow by one token per step",
+            "final_mean_len": float(np.mean(L_end))}
+
+
+def release_all(spk):
+    spk.close()
+    gc.collect()
+    import torch
+    torch.cuda.empty_cache()
+
+
+def headline_line(env: Env, rec, cfg):
+    args = env.args
+    line = {
+        "metric": METRIC, "value": rec["value"], "unit": "GB/s", "n_gpus": env.world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": rec["ms_per_step"], "us_per_step": rec["us_per_step"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+        "config": dict(rec["shape"], workload=rec["workload"], unique_kv_bytes=rec["unique_kv_bytes"],
+                       naive_kv_bytes=rec["naive_kv_bytes"], flops=rec["flops"], l2=L2_NOTE,
+                       parallelism="replicas only" if env.world > 1 else "1 gpu"),
+        "clocks": rec["clocks"], "gpu_launches": int(rec["launches_per_step"] * args.steps),
+        "frac_of_8TBps": rec["frac_of_8TBps"], "frac_of_measured_hbm": rec["frac_of_measured_hbm"],
+        "roofline": rec["roofline"], "e2e": rec["e2e"],
+        "warm_l2_ms_per_step": rec["warm_l2_ms_per_step"], "first_call_us": rec["first_call_us"],
+        "plan_rebuild_us": rec["plan_rebuild_us"], "plan": rec["plan"],
+    }
+    for k in ("verify_tflops", "cpu_baseline", "parity"):
+        if k in rec:
+            line[k] = rec[k]
+    return line
+
+
+def run_single(env: Env, args):
+    """--config 2|3|4|5: one workload, one line (the per-config form of the default run)."""
+    n = int(args.config)
+    cfg = synth.CONFIGS[n]
+    if n == 4:
+        cfg = cfg.scaled(k_draft=args.k)
+    wl = synth.Workload(cfg)
+    num_pages = (1 << 20) if (n == 5 and args.full_pool) else None
+    spk, ids = build_spork(cfg, wl, num_pages, None, env.device)
+    apply_knobs(spk, args)
+    rec = measure_attn(env, spk, ids, cfg, wl)
+    spk.close()
+    return headline_line(env, rec, cfg)
+
+
+def apply_knobs(spk, args):
+    if args.min_rows is not None:
+        spk.set_tensor_path_min_rows(args.min_rows)
+    if args.stream_k is not None:
+        spk.set_stream_k(bool(args.stream_k))
+    if args.many_row_variant is not None:
+        spk.set_many_row_variant(args.many_row_variant)
+
+
+def run_all(env: Env, args):
+    """The default run: config 5 at the top level (the largest single-GPU decode config), everything
+    else under per_config."""
+    t_all = time.perf_counter()
+    per = {}
+    # ---- config 5 on the 2^20-page pool (BASELINE.json configs[4]) + its fork churn: one state ----
+    cfg5 = synth.CFG5
+    wl5 = synth.Workload(cfg5)
+    NP5 = 1 << 20
+    t0 = time.perf_counter()
+    spk, ids = build_spork(cfg5, wl5, NP5, cfg5.n_seqs + 10008, env.device)
+    build5 = time.perf_counter() - t0
+    head = measure_attn(env, spk, ids, cfg5, wl5)
+    head["state_build_seconds"] = build5
+    per["churn"] = measure_churn(env, spk, ids, cfg5, wl5, NP5)
+    release_all(spk)
+    # ---- configs 2 and 3 ----
+    for n in (2, 3):
+        cfg = synth.CONFIGS[n]
+        wl = synth.Workload(cfg)
+        spk, ids = build_spork(cfg, wl, None, None, env.device)
+        per[f"cfg{n}"] = measure_attn(env, spk, ids, cfg, wl)
+        release_all(spk)
+    # ---- config 4: built once with k = 16 drafts per sequence; k = 8 and k = 4 are the same state
+    # rolled back by spork_truncate (the sub-streams make its values identical to a direct build) ----
+    cfg16 = synth.CFG4.scaled(k_draft=16)
+    wl16 = synth.Workload(cfg16)
+    spk, ids = build_spork(cfg16, wl16, None, None, env.device)
+    per["cfg4_k16"] = measure_attn(env, spk, ids, cfg16, wl16)
+    for k in (8, 4):
+        cfgk = synth.CFG4.scaled(k_draft=k)
+        wlk = synth.Workload(cfgk)
+        spk.truncate(ids, wlk.total_len.astype(np.int32))
+        per[f"cfg4_k{k}"] = measure_attn(env, spk, ids, cfgk, wlk)
+    release_all(spk)
+    # ---- the append + decode loop on config 2, and config 1 ----
+    per["loop_cfg2"] = measure_loop(env, synth.CFG2)
+    per["cfg1"] = measure_cfg1(env)
+    line = headline_line(env, head, cfg5)
+    line["config"]["pool_pages"] = NP5
+    line["config"]["state_build_seconds"] = build5
+    line["per_config"] = per
+    line["bench_seconds"] = time.perf_counter() - t_all
+    return line
 
 
 # ---------------------------------------------------------------------------
@@ -557,9 +870,9 @@ def run_d2(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="2", choices=["2", "3", "4", "5", "churn", "d2"])
+    ap.add_argument("--config", default="all", choices=["all", "1", "2", "3", "4", "5", "churn", "loop", "d2"])
     ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-groups", type=int, default=0,
@@ -575,15 +888,43 @@ def main():
     if args.config == "d2":
         run_d2(args)
         return
-    cfg, name = pick_config(args)
-    wl = synth.Workload(cfg)
-    if args.ref_groups <= 0:
-        args.ref_groups = {"2": 16, "3": 8, "4": 2, "5": 4, "churn": 1}[args.config]
     if args.impl == "reference":
-        if int(os.environ.get("RANK", "0")) == 0:
-            run_reference(args, cfg, name, wl)
+        # the oracle on the host cores, on this arm's headline workload (config 5 unless --config says otherwise)
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        n = 5 if args.config in ("all", "churn", "loop") else int(args.config)
+        cfg = synth.CONFIGS[n]
+        if n == 4:
+            cfg = cfg.scaled(k_draft=args.k)
+        print(json.dumps(reference_line(args, cfg, synth.Workload(cfg))))
         return
-    run_ours(args, cfg, name, wl)
+    env = Env(args)
+    if args.config == "all":
+        line = run_all(env, args)
+    elif args.config == "churn":
+        cfg, wl = synth.CFG5, synth.Workload(synth.CFG5)
+        spk, ids = build_spork(cfg, wl, 1 << 20, cfg.n_seqs + 10008, env.device)
+        rec = measure_churn(env, spk, ids, cfg, wl, 1 << 20)
+        spk.close()
+        line = dict(rec, metric="fork_release_churn", n_gpus=env.world, steps=args.steps,
+                    warmup=max(args.warmup, 3), higher_is_better=True, scaling="weak", vs_baseline=None,
+                    data="synthetic", config=dict(rec["shape"], workload=rec["workload"], l2=L2_NOTE),
+                    gpu_launches=int(rec["launches_per_step"] * args.steps))
+    elif args.config == "loop":
+        rec = measure_loop(env, synth.CFG2)
+        line = dict(rec, metric="append_decode_loop_us_per_step", n_gpus=env.world, higher_is_better=True,
+                    scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic",
+                    config={"workload": rec["workload"], "l2": L2_NOTE})
+    elif args.config == "1":
+        rec = measure_cfg1(env)
+        line = dict(rec, metric=METRIC, n_gpus=env.world, steps=args.steps, warmup=max(args.warmup, 3),
+                    higher_is_better=True, scaling="weak", vs_baseline=None, data="synthetic",
+                    config={"workload": rec["workload"]})
+    else:
+        line = run_single(env, args)
+    if env.rank == 0:
+        print(json.dumps(line))
+    env.close()
 
 
 if __name__ == "__main__":

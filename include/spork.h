@@ -27,11 +27,11 @@
  *     from one thread and onto one stream (or onto streams the caller orders).
  *     A handle is not thread-safe.
  *   - Batched state calls are all-or-nothing: on any error no state changes.
- *   - The library never synchronises the stream on the success path, with two
- *     documented exceptions: (a) when its lower bound on free pages cannot
- *     prove that an allocating call fits, it reads the exact device-side free
- *     count (one 4-byte copy); (b) the first attention call after a
- *     fork/release/truncate reads back the per-group shared page counts.
+ *   - The library never synchronises the stream on the success path, with one
+ *     documented exception: when its lower bound on free pages cannot prove
+ *     that an allocating call fits, it reads the exact device-side free count
+ *     (one 4-byte copy).  (Which pages the members of a fork group share is
+ *     known on the host from the fork lineage; nothing is read back for it.)
  *   - Page size is 16 tokens.  Page allocation is deterministic: the lowest
  *     free page id first, requests in array order, positions ascending
  *     (reading A-1), so block tables and refcounts are unique.
@@ -141,10 +141,11 @@ int spork_truncate(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t 
  * decode attention, q_len = 1 (main and probes decode in one
  * batch).  The batch is seq_ids[group_indptr[n_groups]] (host int32), split
  * into fork groups by group_indptr (host int32[n_groups+1]); a group of 1 is
- * plain paged decode.  For each group the library finds the longest run of
- * leading pages common to all members and reads it from HBM once for the
- * whole group (cascade); the result does not depend on the grouping beyond
- * rounding.  q: device [n_seq][Hq][D] cfg.dtype.  out: device fp32
+ * plain paged decode.  For each group the library finds the leading pages
+ * its members have in common -- all of them, and, level by level, every
+ * subset that shares more (probes forked at successive positions) -- and
+ * reads each shared run from HBM once for the members that share it
+ * (cascade); the result does not depend on the grouping beyond rounding.  q: device [n_seq][Hq][D] cfg.dtype.  out: device fp32
  * [n_seq][Hq][D].  lse: device fp32 [n_seq][Hq], natural log of
  * sum_t exp(scale * <q, k_t>).  Row i attends all len(seq_ids[i]) tokens; an
  * empty sequence yields out = 0, lse = -inf.
@@ -207,6 +208,10 @@ typedef struct spork_plan_info {
     int32_t n_umma_items;   /* of n_items, those run by the tcgen05 kernels         */
     int32_t n_two_pipe_items; /* of those, items on the second tcgen05 list (knob)   */
     int32_t stream_k;       /* 1: equal-work contiguous schedule    */
+    float plan_host_us;     /* host time of the last plan BUILD (a cache miss), us   */
+    int32_t plan_builds;    /* plans built on this handle so far (cache misses)      */
+    int32_t n_levels;       /* deepest cascade level of the last plan (1 = single)   */
+    int32_t reserved;
 } spork_plan_info;
 int spork_last_plan(spork_ctx *ctx, spork_plan_info *out);
 /* kernels launched by the last state call (append / fork / release / truncate) */
@@ -215,8 +220,10 @@ int spork_last_launches(spork_ctx *ctx);
 /*
  * Kernel timing for bench.py's roofline: when enabled, the attention calls
  * record CUDA events on `stream` around the attention kernel and around the
- * merge kernel.  spork_last_kernel_ms synchronises on them and returns the two
- * durations of the last call (milliseconds).  Off by default (no events).
+ * merge kernel, and spork_fork records them around fork_clone_kernel (its
+ * dominant kernel; merge_ms is then 0).  spork_last_kernel_ms synchronises on
+ * them and returns the two durations of the last such call (milliseconds).
+ * Off by default (no events).
  */
 int spork_set_timing(spork_ctx *ctx, int enable);
 int spork_last_kernel_ms(spork_ctx *ctx, float *attn_ms, float *merge_ms);
@@ -284,6 +291,42 @@ int spork_set_many_row_variant(spork_ctx *ctx, int mode);
  * beyond rounding.  Invalidates the cached plan.
  */
 int spork_set_stream_k(spork_ctx *ctx, int enable);
+
+/*
+ * Tuning knob: the deepest cascade the planner builds for a fork group (default 7).  A group is
+ * planned as a trie: every set of members that holds further pages in common beyond what the
+ * whole group shares (probes forked from the main stream at successive CoT positions, Algorithm 1
+ * steps 4-6) gets a shared segment of its own, read from HBM once for that set.
+ * max_levels = 1: only the group-wide prefix is shared, deeper sharing is read once per member.
+ * Results do not depend on it beyond rounding.  Invalidates the cached plan.
+ */
+int spork_set_cascade_levels(spork_ctx *ctx, int max_levels);
+
+/*
+ * Multi-layer step (the Qwen3 models the paper serves have 36 / 64 / 48
+ * layers).  Block tables, refcounts and lengths are per SEQUENCE, not per layer: one
+ * handle serves every layer's K/V pools.
+ *   spork_layers: registers the pools of layers 0 .. n_layers-1 (host arrays of device pointers, each
+ *     pool sized and aligned like create's; k_pools[0] / v_pools[0] must be create's pools).  From
+ *     then on spork_fork duplicates a partially filled tail page in EVERY layer.
+ *   spork_append allocates pages and writes layer 0's K/V; spork_write_kv_layer writes the K/V of the
+ *     LAST n_tokens[i] tokens of seq_ids[i] (already appended) into layer `layer`'s pools (k_src,
+ *     v_src: device, [sum n_tokens][Hkv][D]).  Errors: INVALID (n_tokens[i] > len), INVALID_SEQ.
+ *   spork_decode_attn_layers / spork_verify_attn_layers: ONE plan, then n_layers x (attention kernel,
+ *     merge kernel) back to back, layer l on pools l with q[l] -> out[l], lse[l] (HOST arrays of
+ *     n_layers device pointers, shapes as in the single-layer calls).  Each kernel is launched
+ *     programmatically behind the previous one, so launch latency and prologues overlap.  All q[l]
+ *     must be ready when the call is made.
+ */
+int spork_layers(spork_ctx *ctx, int n_layers, void *const *k_pools, void *const *v_pools, void *stream);
+int spork_write_kv_layer(spork_ctx *ctx, int layer, int n, const int32_t *seq_ids, const int32_t *n_tokens,
+                         const void *k_src, const void *v_src, void *stream);
+int spork_decode_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const int32_t *group_indptr,
+                             const int32_t *seq_ids, const void *const *q, float *const *out,
+                             float *const *lse, void *stream);
+int spork_verify_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const int32_t *group_indptr,
+                             const int32_t *seq_ids, const int32_t *q_indptr, const void *const *q,
+                             float *const *out, float *const *lse, void *stream);
 
 const char *spork_strerror(int code);
 

@@ -33,6 +33,8 @@ ABI_SYMBOLS = [
     "spork_decode_attn_host", "spork_verify_attn_host", "spork_export", "spork_export_refcounts",
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
     "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_many_row_variant", "spork_set_stream_k", "spork_strerror",
+    "spork_set_cascade_levels", "spork_layers", "spork_write_kv_layer", "spork_decode_attn_layers",
+    "spork_verify_attn_layers",
 ]
 
 
@@ -47,10 +49,11 @@ class PlanInfo(C.Structure):
                 ("grid", C.c_int32), ("kernel", C.c_int32), ("plan_cached", C.c_int32),
                 ("unique_tokens", C.c_int64), ("naive_tokens", C.c_int64),
                 ("partial_rows", C.c_int64), ("launches", C.c_int32), ("n_umma_items", C.c_int32),
-                ("n_two_pipe_items", C.c_int32), ("stream_k", C.c_int32)]
+                ("n_two_pipe_items", C.c_int32), ("stream_k", C.c_int32), ("plan_host_us", C.c_float),
+                ("plan_builds", C.c_int32), ("n_levels", C.c_int32), ("reserved", C.c_int32)]
 
     def as_dict(self):
-        return {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+        return {k: (float if t is C.c_float else int)(getattr(self, k)) for k, t in self._fields_ if k != "reserved"}
 
 
 _lib = None
@@ -96,6 +99,11 @@ def load(build_if_missing: bool = True):
         "spork_set_tensor_path_min_rows": ([P, I], I),
         "spork_set_many_row_variant": ([P, I], I),
         "spork_set_stream_k": ([P, I], I),
+        "spork_set_cascade_levels": ([P, I], I),
+        "spork_layers": ([P, I, P, P, P], I),
+        "spork_write_kv_layer": ([P, I, I, P, P, P, P, P], I),
+        "spork_decode_attn_layers": ([P, I, I, P, P, P, P, P, P], I),
+        "spork_verify_attn_layers": ([P, I, I, P, P, P, P, P, P, P], I),
         "spork_last_kernel_ms": ([P, P, P], I),
         "spork_strerror": ([I], C.c_char_p),
     }
@@ -182,6 +190,14 @@ class Spork:
         if cur != self.stream:
             cur.wait_stream(self.stream)
 
+    def _hold(self, *tensors):
+        """caller tensors are read on OUR stream: tell the caching allocator, so that memory freed on the
+        caller's stream is not reused before our kernels have read it"""
+        for t in tensors:
+            if t is not None and t.is_cuda:
+                t.record_stream(self.stream)
+        self._keep = tensors
+
     @staticmethod
     def _chk(rc: int, check: bool = True) -> int:
         if rc != OK and check:
@@ -209,7 +225,7 @@ class Spork:
         assert kd.numel() * kd.element_size() == total * self.Hkv * self.D * (4 if self.dtype == "f32" else 2)
         self._enter()
         rc = self.lib.spork_append(self._h, len(s), _p(s), _p(nt), kd.data_ptr(), vd.data_ptr(), self._st)
-        self._keep = (kd, vd)   # stream-ordered use: keep alive until the next call
+        self._hold(kd, vd)
         return self._chk(rc, check)
 
     def fork(self, parents, check: bool = True):
@@ -235,9 +251,11 @@ class Spork:
         t = target_tokens if hasattr(target_tokens, "data_ptr") else self._dev(np.asarray(target_tokens, dtype=np.int32))
         assert d.dtype == torch.int32 and t.dtype == torch.int32
         acc = np.zeros(len(s), np.int32)
-        rc = self._chk(self.lib.spork_accept(self._h, len(s), _p(s), _p(qi), C.c_void_p(d.data_ptr()),
-                                             C.c_void_p(t.data_ptr()), _p(acc), self._st), check)
-        return rc, acc
+        self._enter()            # drafts / targets may have been produced on torch's current stream
+        rc = self.lib.spork_accept(self._h, len(s), _p(s), _p(qi), C.c_void_p(d.data_ptr()),
+                                   C.c_void_p(t.data_ptr()), _p(acc), self._st)
+        self._hold(d, t)
+        return self._chk(rc, check), acc
 
     def confidence(self, span_indptr, logits, out=None, check: bool = True):
         """Eq. 2 confidence per span.  logits: device fp32 tensor [n_pos][vocab] (or numpy).  Returns a
@@ -249,8 +267,12 @@ class Spork:
         n = len(sp) - 1
         if out is None:
             out = torch.empty((n,), dtype=torch.float32, device=self.device)
-        rc = self._chk(self.lib.spork_confidence(self._h, n, _p(sp), C.c_void_p(x.data_ptr()), int(x.shape[1]),
-                                                 C.c_void_p(out.data_ptr()), self._st), check)
+        self._enter()            # the logits may still be in flight on torch's current stream
+        rc = self.lib.spork_confidence(self._h, n, _p(sp), C.c_void_p(x.data_ptr()), int(x.shape[1]),
+                                       C.c_void_p(out.data_ptr()), self._st)
+        self._leave()            # ... and the scores are read there
+        self._hold(x, out)
+        self._chk(rc, check)
         return out if check else (rc, out)
 
     # ---- attention ------------------------------------------------------------
@@ -269,7 +291,7 @@ class Spork:
         rc = self.lib.spork_decode_attn(self._h, len(gi) - 1, _p(gi), _p(s), qd.data_ptr(),
                                         out.data_ptr(), lse.data_ptr(), self._st)
         self._leave()
-        self._keep = (qd,)
+        self._hold(qd, out, lse)
         self._chk(rc, check)
         return (out, lse) if check else (rc, out, lse)
 
@@ -286,9 +308,51 @@ class Spork:
         rc = self.lib.spork_verify_attn(self._h, len(gi) - 1, _p(gi), _p(s), _p(qi), qd.data_ptr(),
                                         out.data_ptr(), lse.data_ptr(), self._st)
         self._leave()
-        self._keep = (qd,)
+        self._hold(qd, out, lse)
         self._chk(rc, check)
         return (out, lse) if check else (rc, out, lse)
+
+    # ---- multi-layer step -------------------------------------
+    def layers(self, n_layers: int):
+        """Allocates and registers the K/V pools of layers 1 .. n_layers-1 (layer 0 = the pools made at
+        construction); block tables, refcounts and lengths are shared by all layers."""
+        torch = self.torch
+        self.k_pools = [self.k_pool] + [torch.empty_like(self.k_pool) for _ in range(n_layers - 1)]
+        self.v_pools = [self.v_pool] + [torch.empty_like(self.v_pool) for _ in range(n_layers - 1)]
+        kp = (C.c_void_p * n_layers)(*[t.data_ptr() for t in self.k_pools])
+        vp = (C.c_void_p * n_layers)(*[t.data_ptr() for t in self.v_pools])
+        self._chk(self.lib.spork_layers(self._h, n_layers, kp, vp, self._st))
+        self.n_layers = n_layers
+
+    def write_kv_layer(self, layer: int, seq_ids, n_tokens, k, v, check: bool = True) -> int:
+        """K/V of the last n_tokens[i] tokens of each sequence into layer `layer`'s pools."""
+        s, nt = _i32(seq_ids), _i32(n_tokens)
+        kd = k if hasattr(k, "data_ptr") else self._dev(np.asarray(k, dtype=self.np_dtype))
+        vd = v if hasattr(v, "data_ptr") else self._dev(np.asarray(v, dtype=self.np_dtype))
+        self._enter()
+        rc = self.lib.spork_write_kv_layer(self._h, int(layer), len(s), _p(s), _p(nt), kd.data_ptr(),
+                                           vd.data_ptr(), self._st)
+        self._hold(kd, vd)
+        return self._chk(rc, check)
+
+    def attn_layers(self, group_indptr, seq_ids, q_layers, out_layers, lse_layers, q_indptr=None):
+        """One plan, len(q_layers) x (attention, merge) launches back to back.  q_layers / out_layers /
+        lse_layers: lists of device tensors, one per layer."""
+        gi, s = _i32(group_indptr), _i32(seq_ids)
+        L = len(q_layers)
+        qp = (C.c_void_p * L)(*[t.data_ptr() for t in q_layers])
+        op = (C.c_void_p * L)(*[t.data_ptr() for t in out_layers])
+        lp = (C.c_void_p * L)(*[t.data_ptr() for t in lse_layers])
+        self._enter()
+        if q_indptr is None:
+            rc = self.lib.spork_decode_attn_layers(self._h, L, len(gi) - 1, _p(gi), _p(s), qp, op, lp, self._st)
+        else:
+            qi = _i32(q_indptr)
+            rc = self.lib.spork_verify_attn_layers(self._h, L, len(gi) - 1, _p(gi), _p(s), _p(qi), qp, op, lp,
+                                                   self._st)
+        self._leave()
+        self._hold(*q_layers, *out_layers, *lse_layers)
+        self._chk(rc)
 
     def decode_attn_host(self, group_indptr, seq_ids, q_host, out_host, lse_host):
         """HOST (pinned) tensors in, HOST tensors out; copies run inside the call."""
@@ -347,9 +411,15 @@ class Spork:
         """Planner knob: segments with >= min_rows rows per KV head run on the tcgen05 kernel."""
         self._chk(self.lib.spork_set_tensor_path_min_rows(self._h, int(min_rows)))
 
-    def set_many_row_variant(self, enable: bool):
-        """Planner knob: run > 128-row segments on the two-pipe tcgen05 kernel (default on)."""
-        self._chk(self.lib.spork_set_many_row_variant(self._h, int(enable)))
+    def set_many_row_variant(self, mode: int):
+        """Planner knob: which tcgen05 kernel runs segments of more than 128 rows.  0 (default): the
+        one-pipe kernel in row blocks of 128; 1: the two-pipe kernel (row blocks of 256 over one K/V
+        stream); 2: the split-row kernel."""
+        self._chk(self.lib.spork_set_many_row_variant(self._h, int(mode)))
+
+    def set_cascade_levels(self, max_levels: int):
+        """Planner knob: deepest cascade built for a fork group (1: the group-wide prefix only)."""
+        self._chk(self.lib.spork_set_cascade_levels(self._h, int(max_levels)))
 
     def set_stream_k(self, enable: bool):
         """Planner knob: equal-work contiguous schedule for single-row-block calls (default on)."""

@@ -192,7 +192,7 @@ struct ParentDesc {
 __global__ void __launch_bounds__(256) fork_clone_kernel(
     const ForkDesc *__restrict__ descs, const int32_t *__restrict__ free_list, int32_t *table,
     int table_stride, int32_t *len, int32_t *refcount, uint8_t *k_pool, uint8_t *v_pool,
-    size_t page_bytes, int32_t *counters, int need) {
+    size_t page_bytes, int32_t *counters, int need, int n_extra_pools, uint8_t *const *extra_pools) {
     __shared__ int s_tail;
     ForkDesc d = descs[blockIdx.x];
     int nf = d.len / PS;
@@ -230,6 +230,12 @@ __global__ void __launch_bounds__(256) fork_clone_kernel(
     for (size_t j = threadIdx.x; j < n16; j += blockDim.x) {
         kd[j] = ks[j];
         vd[j] = vs[j];
+    }
+    // the other layers' pools (spork_layers): block tables are shared, so the tail is duplicated in each
+    for (int e = 0; e < n_extra_pools; ++e) {
+        const uint4 *src2 = reinterpret_cast<const uint4 *>(extra_pools[e] + (size_t)s_tail * page_bytes);
+        uint4 *dst2 = reinterpret_cast<uint4 *>(extra_pools[e] + (size_t)tail_page * page_bytes);
+        for (size_t j = threadIdx.x; j < n16; j += blockDim.x) dst2[j] = src2[j];
     }
 }
 
@@ -397,6 +403,7 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
         tok += n_tokens[i];
         foff += d[i].n_new;
         c->h_len[s] = nl;
+        lineage_grow(c, s, pages_of(nl));
     }
     rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
     if (rc != SPORK_OK) return rc;
@@ -419,6 +426,48 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
     SPORK_CUDA(cudaGetLastError());
     c->free_lb -= need;
     c->len_epoch++;
+    return stage_done(c, slot, st);
+}
+
+// K/V of the LAST n_tokens[i] tokens of each sequence into another layer's pools:
+// the pages were allocated by spork_append (block tables are shared by all layers)
+extern "C" int spork_write_kv_layer(spork_ctx *c, int layer, int n, const int32_t *seq_ids,
+                                    const int32_t *n_tokens, const void *k_src, const void *v_src, void *stream) {
+    if (!c || n < 0 || (n > 0 && (!seq_ids || !n_tokens))) return SPORK_ERR_INVALID;
+    if (layer < 0 || layer > (int)c->layer_k.size()) return SPORK_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    c->last_launches = 0;
+    if (n == 0) return SPORK_OK;
+    int64_t total = 0;
+    for (int i = 0; i < n; ++i) {
+        const int s = seq_ids[i];
+        if (s < 0 || s >= c->cfg.max_seqs || !c->h_live[s]) return SPORK_ERR_INVALID_SEQ;
+        if (n_tokens[i] < 0 || n_tokens[i] > c->h_len[s]) return SPORK_ERR_INVALID;
+        total += n_tokens[i];
+    }
+    if (total == 0) return SPORK_OK;
+    if (!k_src || !v_src || total >= (int64_t)1 << 31) return SPORK_ERR_INVALID;
+    StageSlot *slot;
+    int rc = stage_acquire(c, sizeof(AppendDesc) * (size_t)n, &slot);
+    if (rc != SPORK_OK) return rc;
+    AppendDesc *d = (AppendDesc *)slot->h;
+    int tok = 0;
+    for (int i = 0; i < n; ++i) {
+        d[i] = AppendDesc{seq_ids[i], c->h_len[seq_ids[i]] - n_tokens[i], n_tokens[i], tok, 0, 0, -1, 0};
+        tok += n_tokens[i];
+    }
+    rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
+    if (rc != SPORK_OK) return rc;
+    const int cpr = c->cfg.head_dim * c->elt / 16;
+    const size_t units = (size_t)total * c->cfg.num_kv_heads * cpr;
+    const int blocks = (int)std::min<size_t>((units + 255) / 256, (size_t)c->num_sms * 16);
+    uint8_t *kp = (uint8_t *)(layer == 0 ? c->k_pool : c->layer_k[layer - 1]);
+    uint8_t *vp = (uint8_t *)(layer == 0 ? c->v_pool : c->layer_v[layer - 1]);
+    append_copy_kernel<<<blocks, 256, 0, st>>>((const AppendDesc *)slot->d, n, (const uint4 *)k_src,
+                                               (const uint4 *)v_src, kp, vp, c->d_table, c->table_stride,
+                                               c->cfg.num_kv_heads, cpr, c->swizzled, c->head_block, units);
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
     return stage_done(c, slot, st);
 }
 
@@ -470,6 +519,7 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
         c->h_shared_upto[p] = std::max(c->h_shared_upto[p], L / PS);
         c->h_fork_key[s] = (c->fork_calls << 32) | (uint64_t)(p + 1);   // same call, same parent: same prefix
         c->h_fork_nf[s] = L / PS;
+        lineage_fork(c, s, p, L);
         fd[i].parent = p;
         fd[i].child = s;
         fd[i].len = L;
@@ -488,11 +538,18 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
                                                    c->d_table, c->table_stride, c->d_refcount);
         c->last_launches++;
     }
+    if (c->timing) SPORK_CUDA(cudaEventRecord(c->t_ev[0], st));
     fork_clone_kernel<<<n, 256, 0, st>>>((const ForkDesc *)slot->d, c->d_free_list, c->d_table,
                                          c->table_stride, c->d_len, c->d_refcount,
                                          (uint8_t *)c->k_pool, (uint8_t *)c->v_pool, c->page_bytes,
-                                         c->d_counters, (int)need);
+                                         c->d_counters, (int)need, (int)(c->layer_k.size() * 2),
+                                         (uint8_t *const *)c->d_layer_pools.p);
     c->last_launches++;
+    if (c->timing) {
+        SPORK_CUDA(cudaEventRecord(c->t_ev[1], st));
+        SPORK_CUDA(cudaEventRecord(c->t_ev[2], st));
+        c->t_valid = true;
+    }
     SPORK_CUDA(cudaGetLastError());
     c->free_lb -= need;
     c->structure_epoch++;
@@ -588,11 +645,13 @@ static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_
             c->h_len[s] = new_len[i];
             c->h_shared_upto[s] = std::min(c->h_shared_upto[s], pages_of(new_len[i]));
             c->h_fork_key[s] = 0;      // a rolled-back sequence no longer mirrors its siblings
+            lineage_truncate(c, s, pages_of(new_len[i]));
         } else {
             c->h_len[s] = 0;
             c->h_live[s] = 0;
             c->h_shared_upto[s] = 0;
             c->h_fork_key[s] = 0;
+            lineage_reset(c, s);
         }
     }
     if (!new_len) c->n_live -= n;

@@ -126,14 +126,14 @@ extern "C" int spork_create(const spork_config *cfg, void *k_pool, void *v_pool,
     c->free_lb = cfg->num_pages;
     c->n_live = 0;
     c->last_launches = 0;
-    c->plan_ev = nullptr;
-    c->plan_ev_pending = false;
     c->h_len.assign(cfg->max_seqs, 0);
     c->h_live.assign(cfg->max_seqs, 0);
     c->h_shared_upto.assign(cfg->max_seqs, 0);
     c->h_fork_key.assign(cfg->max_seqs, 0);
     c->h_fork_nf.assign(cfg->max_seqs, 0);
     c->h_scratch.assign(cfg->max_seqs, 0);
+    c->h_lin.assign(cfg->max_seqs, Lineage{});
+    c->h_uid.assign(cfg->max_seqs, 0);
 
     int dev = 0;
     bool ok = cudaGetDevice(&dev) == cudaSuccess &&
@@ -147,7 +147,6 @@ extern "C" int spork_create(const spork_config *cfg, void *k_pool, void *v_pool,
     ok = ok && cudaMalloc(&c->d_counters, 16 * 4) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_free_list, c->free_list_cap * 4) == cudaSuccess;
     ok = ok && cudaMalloc(&c->d_scan, (size_t)(scan_blocks + 1) * 4) == cudaSuccess;
-    ok = ok && cudaEventCreateWithFlags(&c->plan_ev, cudaEventDisableTiming) == cudaSuccess;
     if (ok) {
         init_state_kernel<<<256, 256>>>(c->d_refcount, cfg->num_pages, c->d_table, n_table, c->d_len,
                                         cfg->max_seqs, c->d_counters);
@@ -175,10 +174,9 @@ extern "C" int spork_destroy(spork_ctx *c) {
         if (s.d) cudaFree(s.d);
         if (s.ev) cudaEventDestroy(s.ev);
     }
-    for (DevBuf *b : {&c->plan.items, &c->plan.qdesc, &c->plan.streams, &c->plan.cta_ptr, &c->ws_o, &c->ws_lse, &c->ws_conf, &c->conf_desc, &c->io_q, &c->io_out,
-                      &c->io_lse})
+    for (DevBuf *b : {&c->plan.blob, &c->ws_o, &c->ws_lse, &c->ws_conf, &c->conf_desc, &c->io_q, &c->io_out, &c->io_lse,
+                      &c->d_layer_pools})
         if (b->p) cudaFree(b->p);
-    if (c->plan_ev) cudaEventDestroy(c->plan_ev);
     for (auto &e : c->t_ev)
         if (e) cudaEventDestroy(e);
     delete c;
@@ -197,6 +195,7 @@ extern "C" int spork_seq_create(spork_ctx *c, int n, int32_t *ids_out) {
             c->h_len[s] = 0;
             c->h_shared_upto[s] = 0;
             c->h_fork_key[s] = 0;
+            lineage_reset(c, s);
             ids_out[i++] = s;
         }
     c->n_live += n;

@@ -92,6 +92,8 @@ __device__ __forceinline__ void consumer_bar() {   // the 4 consumer warps only
 struct Params {
     const WorkItem *items;
     const int32_t *cta_ptr;       // this CTA runs items [cta_ptr[b], cta_ptr[b + 1])
+    const int32_t *seq_len;       // device lengths: open-ended items end there
+    const int32_t *rowmap;
     const uint16_t *q;
     const uint8_t *k_pool, *v_pool;
     const int32_t *table;
@@ -255,7 +257,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
     if (warp == N_CONSUMER_WARPS) {
         // ============================ producer ============================
         for (int idx = item_begin; idx < item_end; ++idx) {
-            const WorkItem it = P.items[idx];
+            const WorkItem it = load_item(P.items, idx, P.seq_len);
             const int page0 = it.tok0 / PS;
             const int n_pages = (it.tok1 + PS - 1) / PS - page0;
             const int n_tiles = (n_pages + TILE_PAGES - 1) / TILE_PAGES;
@@ -299,7 +301,7 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
     // ================================ consumers ================================
     const int g = lane >> 2, tq = (lane & 3) * 2;
     for (int idx = item_begin; idx < item_end; ++idx) {
-        const WorkItem it = P.items[idx];
+        const WorkItem it = load_item(P.items, idx, P.seq_len);
         const int RT = it.nrows <= 16 ? 1 : (it.nrows <= 32 ? 2 : 4);   // row tiles of 16
         const int TP = N_CONSUMER_WARPS / RT;                             // token parts of a tile
         const int rt = warp % RT, tp = warp / RT;
@@ -313,12 +315,12 @@ __global__ void __launch_bounds__(N_THREADS, CTAS_PER_SM) attn_mma_kernel(const 
             const uint16_t *q0 = nullptr, *q1 = nullptr;
             if (rr0 < it.nrows) {
                 const int lr = it.rb0 + rr0;
-                q0 = P.q + ((size_t)(it.qrow0 + lr / P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D;
+                q0 = P.q + ((size_t)item_qrow(it, P.rowmap, lr, P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D;
                 lim_r0 = it.lim0 + lr / P.G;
             }
             if (rr1 < it.nrows) {
                 const int lr = it.rb0 + rr1;
-                q1 = P.q + ((size_t)(it.qrow0 + lr / P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D;
+                q1 = P.q + ((size_t)item_qrow(it, P.rowmap, lr, P.G) * P.Hq + it.kvh * P.G + lr % P.G) * D;
                 lim_r1 = it.lim0 + lr / P.G;
             }
 #pragma unroll
@@ -446,21 +448,22 @@ namespace spork {
 
 int attn_mma_grid(spork_ctx *c) { return c->num_sms * CTAS_PER_SM; }
 
-int launch_attn_mma(spork_ctx *c, const void *q, bool programmatic, cudaStream_t st) {
+int launch_attn_mma(spork_ctx *c, const LayerIO &io, bool programmatic, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_items == 0) return SPORK_OK;
-    static bool attr_set = false;
-    if (!attr_set) {
+    if (!(c->smem_attr_done & 8u)) {       // per handle (= per device), not per process
         SPORK_CUDA(cudaFuncSetAttribute(attn_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         SMEM_BYTES));
-        attr_set = true;
+        c->smem_attr_done |= 8u;
     }
     Params p;
-    p.items = (const WorkItem *)P.items.p;
-    p.cta_ptr = (const int32_t *)P.cta_ptr.p;
-    p.q = (const uint16_t *)q;
-    p.k_pool = (const uint8_t *)c->k_pool;
-    p.v_pool = (const uint8_t *)c->v_pool;
+    p.items = P.d_items;
+    p.cta_ptr = P.d_cta_ptr;
+    p.seq_len = c->d_len;
+    p.rowmap = P.d_rowmap;
+    p.q = (const uint16_t *)io.q;
+    p.k_pool = (const uint8_t *)io.k_pool;
+    p.v_pool = (const uint8_t *)io.v_pool;
     p.table = c->d_table;
     p.table_stride = c->table_stride;
     p.Hq = c->cfg.num_q_heads;

@@ -59,12 +59,13 @@ __device__ __forceinline__ float warp_sum(float v) {
 
 template <typename T, int DMAX>
 __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
-    const WorkItem *__restrict__ items, const T *__restrict__ q, const uint8_t *__restrict__ k_pool,
+    const WorkItem *__restrict__ items, const int32_t *__restrict__ seq_len,
+    const int32_t *__restrict__ rowmap, const T *__restrict__ q, const uint8_t *__restrict__ k_pool,
     const uint8_t *__restrict__ v_pool, const int32_t *__restrict__ table, int table_stride, int Hq,
     int Hkv, int G, int D, int swizzled, float scale, float *__restrict__ ws_o,
     float *__restrict__ ws_lse) {
     __shared__ float qs[SIMT_WARPS][DMAX];
-    const WorkItem it = items[blockIdx.x];
+    const WorkItem it = load_item(items, blockIdx.x, seq_len);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     constexpr int E = Elt<T>::PER_CHUNK;
     const int cpr = D / E;                       // 16-byte chunks per row
@@ -74,7 +75,7 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
 
     for (int r = warp; r < it.nrows; r += SIMT_WARPS) {
         const int lr = it.rb0 + r;
-        const int qrow = it.qrow0 + lr / G, h = it.kvh * G + lr % G;
+        const int qrow = item_qrow(it, rowmap, lr, G), h = it.kvh * G + lr % G;
         const int lim = it.lim0 + lr / G;
         __syncwarp();
         for (int d = lane; d < D; d += 32)
@@ -147,6 +148,7 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
 // every load of a batch in flight before the first use (the kernel is pure L2 latency).
 template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
 __global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__ qd,
+                                                    const RowRef *__restrict__ refs,
                                                     const StreamDesc *__restrict__ streams, int n_qrows, int Hq,
                                                     int G, int D, const float *ws_o, const float *ws_lse,
                                                     float *__restrict__ out, float *__restrict__ lse) {
@@ -155,13 +157,15 @@ __global__ void __launch_bounds__(128) merge_kernel(const QRowDesc *__restrict__
     if (w >= n_qrows * Hq) return;
     const int qrow = w / Hq, h = w % Hq;
     const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
-    const RowStreams rs = load_row_streams(streams, d, h / G);
+    const RowSplits rs = load_row_splits(d, refs, streams, h / G, lane);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // a next layer's attention kernel may queue up
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    merge_row<NI>(rs, d, h % G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
+    merge_row<NI>(rs, h % G, D, ws_o, ws_lse, out + (size_t)w * D, lse + w, lane);
 }
 
 template <int NI>
 __global__ void __launch_bounds__(128) merge_heads_kernel(const QRowDesc *__restrict__ qd,
+                                                          const RowRef *__restrict__ refs,
                                                           const StreamDesc *__restrict__ streams, int n_qrows,
                                                           int Hq, int G, int D, const float *ws_o,
                                                           const float *ws_lse, float *__restrict__ out,
@@ -173,40 +177,41 @@ __global__ void __launch_bounds__(128) merge_heads_kernel(const QRowDesc *__rest
     if (w >= n_qrows * Hkv) return;
     const int qrow = w / Hkv, kvh = w % Hkv;
     const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
-    const RowStreams rs = load_row_streams(streams, d, kvh);
+    const RowSplits rs = load_row_splits(d, refs, streams, kvh, lane);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const size_t row0 = (size_t)qrow * Hq + (size_t)kvh * G;
     constexpr int JB = NI == 1 ? 8 : 4;
     int j = 0;
     for (; j + JB <= G; j += JB)
-        merge_heads<NI, JB>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        merge_heads<NI, JB>(rs, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
     if (G - j >= 4 && JB > 4) {
-        merge_heads<NI, 4>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        merge_heads<NI, 4>(rs, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
         j += 4;
     }
     if (G - j >= 2) {
-        merge_heads<NI, 2>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        merge_heads<NI, 2>(rs, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
         j += 2;
     }
     for (; j < G; ++j)
-        merge_row<NI>(rs, d, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
+        merge_row<NI>(rs, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
 }
 
 }  // namespace
 
 namespace spork {
 
-int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st) {
+int launch_attn_simt(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_items == 0) return SPORK_OK;
-    const WorkItem *items = (const WorkItem *)P.items.p;
+    const WorkItem *items = P.d_items;
     float *wo = (float *)c->ws_o.p, *wl = (float *)c->ws_lse.p;
-    const uint8_t *kp = (const uint8_t *)c->k_pool, *vp = (const uint8_t *)c->v_pool;
+    const uint8_t *kp = (const uint8_t *)io.k_pool, *vp = (const uint8_t *)io.v_pool;
     const spork_config &f = c->cfg;
     dim3 grid(P.n_items), block(SIMT_WARPS * 32);
 #define SPORK_SIMT(T, DMAX)                                                                        \
-    attn_simt_kernel<T, DMAX><<<grid, block, 0, st>>>(items, (const T *)q, kp, vp, c->d_table,     \
-                                                      c->table_stride, f.num_q_heads,              \
+    attn_simt_kernel<T, DMAX><<<grid, block, 0, st>>>(items, c->d_len, P.d_rowmap, (const T *)io.q, kp, vp, \
+                                                      c->d_table, c->table_stride, f.num_q_heads,  \
                                                       f.num_kv_heads, c->G, f.head_dim,            \
                                                       c->swizzled, f.scale, wo, wl)
     if (f.dtype == SPORK_F32) {
@@ -224,7 +229,7 @@ int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st) {
     return SPORK_OK;
 }
 
-int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
+int launch_merge(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
     const Plan &P = c->plan;
     if (P.n_qrows == 0) return SPORK_OK;
     // enough (q row, kv head) pairs to fill the SMs: the grouped kernel (measured: verify k = 16 merge
@@ -242,10 +247,10 @@ int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st) {
     cfg.numAttrs = 1;
     auto kern = grouped ? (c->cfg.head_dim <= 128 ? merge_heads_kernel<1> : merge_heads_kernel<2>)
                         : (c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>);
-    SPORK_CUDA(cudaLaunchKernelEx(&cfg, kern,
-                                  (const QRowDesc *)P.qdesc.p, (const StreamDesc *)P.streams.p, P.n_qrows,
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, kern, P.d_qdesc, P.d_refs, P.d_streams, P.n_qrows,
                                   (int)c->cfg.num_q_heads, c->G, (int)c->cfg.head_dim,
-                                  (const float *)c->ws_o.p, (const float *)c->ws_lse.p, out, lse));
+                                  (const float *)c->ws_o.p, (const float *)c->ws_lse.p,
+                                  io.out, io.lse));
     c->last_launches++;
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;

@@ -74,12 +74,16 @@ enum : int {
 struct UParams {
     const WorkItem *items;
     const int32_t *cta_ptr;
+    const int32_t *seq_len;       // device lengths: open-ended items end there
+    const int32_t *rowmap;
     const uint16_t *q;
     const uint8_t *k_pool, *v_pool;
     const int32_t *table;
     int table_stride, Hq, Hkv, G;
     float scale_log2;
     float *ws_o, *ws_lse;
+    int wait_prev;                // launched programmatically behind a kernel that still READS ws_o / ws_lse
+                                  // (the merge of the previous layer): wait for it before the first partial
 };
 
 template <int NP, int SP>
@@ -129,7 +133,7 @@ attn_umma_kernel(const UParams P) {
         // ================================ producer ================================
         uint32_t ld = 0;   // loads issued so far: slot = ld % NSLOT, phase = (ld / NSLOT) & 1
         for (int idx = item_begin; idx < item_end; ++idx) {
-            const WorkItem it = P.items[idx];
+            const WorkItem it = load_item(P.items, idx, P.seq_len);
             const int page0 = it.tok0 / PS;
             const int n_pages = (it.tok1 + PS - 1) / PS - page0;
             const int n_tiles = (n_pages + TILE_PAGES - 1) / TILE_PAGES;
@@ -183,7 +187,7 @@ attn_umma_kernel(const UParams P) {
         for (int w = 0; w < NP; ++w) { g0[w] = 0; jw[w] = 0; }
         int j = 0;
         for (int idx = item_begin; idx < item_end; ++idx, ++j) {
-            const WorkItem it = P.items[idx];
+            const WorkItem it = load_item(P.items, idx, P.seq_len);
             const int n_tok = it.tok1 - it.tok0;
             const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
             const int npipe = (NP > 1 && it.nrows > 128) ? 2 : 1;   // pipe 1 sits idle on a <= 128-row item
@@ -276,7 +280,7 @@ attn_umma_kernel(const UParams P) {
                 if (row < qi.nrows) {
                     const int lr = qi.rb0 + row;
                     const uint16_t *src =
-                        P.q + ((size_t)(qi.qrow0 + lr / P.G) * P.Hq + qi.kvh * P.G + lr % P.G) * D + c * 8;
+                        P.q + ((size_t)item_qrow(qi, P.rowmap, lr, P.G) * P.Hq + qi.kvh * P.G + lr % P.G) * D + c * 8;
                     v[k] = *reinterpret_cast<const uint4 *>(src);
                 }
             }
@@ -293,7 +297,7 @@ attn_umma_kernel(const UParams P) {
         };
         if (item_begin < item_end) stage_q(P.items[item_begin]);
         for (int idx = item_begin; idx < item_end; ++idx) {
-            const WorkItem it = P.items[idx];
+            const WorkItem it = load_item(P.items, idx, P.seq_len);
             const bool has_next = idx + 1 < item_end;
             const int n_tok = it.tok1 - it.tok0;
             const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
@@ -426,6 +430,7 @@ attn_umma_kernel(const UParams P) {
                     pair_sync();                                   // ... before the next item's first tile
                     const float inv = lr > 0.f ? 1.f / lr : 0.f;
                     float *dst = P.ws_o + (size_t)(it.part_base + r) * D;
+                    if (P.wait_prev && idx == item_begin) asm volatile("griddepcontrol.wait;" ::: "memory");
 #pragma unroll 1
                     for (int cb = 2 * h; cb < 2 * h + 2; ++cb) {
                         uint32_t o[32];
@@ -559,6 +564,7 @@ attn_umma_kernel(const UParams P) {
                 tc_fence_after();
                 const float inv = lr > 0.f ? 1.f / lr : 0.f;
                 float *dst = P.ws_o + (size_t)(it.part_base + r) * D;
+                if (P.wait_prev && idx == item_begin) asm volatile("griddepcontrol.wait;" ::: "memory");
 #pragma unroll 1
                 for (int cb = 0; cb < 4; ++cb) {
                     uint32_t o[32];
@@ -608,11 +614,11 @@ int attn_umma_grid(spork_ctx *c, int variant) {
 
 template <int NP, int SP>
 static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic, cudaStream_t st) {
-    static bool attr_set = false;
-    if (!attr_set) {
+    constexpr uint32_t bit = 1u << (NP == 2 ? 1 : (SP == 2 ? 2 : 0));
+    if (!(c->smem_attr_done & bit)) {      // per handle (= per device), not per process
         SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         Cfg<NP, SP>::SMEM_BYTES));
-        attr_set = true;
+        c->smem_attr_done |= bit;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
@@ -623,7 +629,7 @@ static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = programmatic ? 1 : 0;   // may start while the previous attention kernel drains
+    cfg.numAttrs = programmatic ? 1 : 0;   // may start while the previous kernel drains
     SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP, SP>, p));
     c->last_launches++;
     SPORK_CUDA(cudaGetLastError());
@@ -631,17 +637,19 @@ static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic
 }
 
 // np = 2: the many-row items' list (launched first; two-pipe or split-row kernel), np = 1: the others
-int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st) {
+int launch_attn_umma(spork_ctx *c, const LayerIO &io, int np, bool programmatic, bool wait_prev, cudaStream_t st) {
     const Plan &P = c->plan;
     const int n = np == 2 ? P.n_items_umma2 : P.n_items_umma;
     if (n == 0) return SPORK_OK;
     UParams p;
     // item lists: [mma.sync][tcgen05 NP=1][tcgen05 NP=2]; cta_ptr arrays in the same order
-    p.items = (const WorkItem *)P.items.p + P.n_items + (np == 2 ? P.n_items_umma : 0);
-    p.cta_ptr = (const int32_t *)P.cta_ptr.p + (P.grid + 1) + (np == 2 ? P.grid_umma + 1 : 0);
-    p.q = (const uint16_t *)q;
-    p.k_pool = (const uint8_t *)c->k_pool;
-    p.v_pool = (const uint8_t *)c->v_pool;
+    p.items = P.d_items + P.n_items + (np == 2 ? P.n_items_umma : 0);
+    p.cta_ptr = P.d_cta_ptr + (P.grid + 1) + (np == 2 ? P.grid_umma + 1 : 0);
+    p.seq_len = c->d_len;
+    p.rowmap = P.d_rowmap;
+    p.q = (const uint16_t *)io.q;
+    p.k_pool = (const uint8_t *)io.k_pool;
+    p.v_pool = (const uint8_t *)io.v_pool;
     p.table = c->d_table;
     p.table_stride = c->table_stride;
     p.Hq = c->cfg.num_q_heads;
@@ -650,6 +658,7 @@ int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cud
     p.scale_log2 = c->cfg.scale * LOG2E;
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
+    p.wait_prev = wait_prev ? 1 : 0;
     if (np == 1) return launch_np<1, 1>(c, p, P.grid_umma, programmatic, st);
     return P.variant2 == 2 ? launch_np<1, 2>(c, p, P.grid_umma2, programmatic, st)
                            : launch_np<2, 1>(c, p, P.grid_umma2, programmatic, st);

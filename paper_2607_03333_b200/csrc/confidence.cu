@@ -6,8 +6,11 @@
 //                         (max, sum of exp relative to that max), 16-byte loads, 8 values per
 //                         rescale of the running sum
 //   conf_span_kernel    : one warp per span combines the slices of each row and takes the minimum
+#include <limits.h>
 #include <math.h>
 #include <string.h>
+
+#include <algorithm>
 
 #include "spork_internal.h"
 
@@ -49,13 +52,15 @@ __device__ __forceinline__ void combine(float &m, float &s, float m2, float s2) 
 }
 
 __global__ void __launch_bounds__(THREADS) conf_partial_kernel(const float *__restrict__ logits, int vocab,
-                                                               int chunk, const int32_t *__restrict__ rows,
+                                                               int chunk, int splits, int vec,
+                                                               const int32_t *__restrict__ rows,
                                                                float2 *__restrict__ part) {
-    const int row = rows[blockIdx.y], sx = blockIdx.x;      // only rows i >= 2 of their span are read
+    // grid.x = rows x splits (a 1-D grid: no 65,535 limit on the row count)
+    const int row = rows[blockIdx.x / splits], sx = blockIdx.x % splits;   // only rows i >= 2 of their span are read
     const float *x = logits + (size_t)row * vocab;
     const int v0 = sx * chunk, v1 = min(vocab, v0 + chunk);
     float m = -INFINITY, s = 0.f;
-    const bool vec = (vocab & 3) == 0;   // rows 16-byte aligned (chunk is a multiple of 8)
+    // vec: every row is 16-byte aligned (vocab % 4 == 0 and an aligned base; chunk is a multiple of 8)
     if (vec) {
         // 4 batches of 8 values (8 x 16-byte loads) in flight per thread before the first exp
         constexpr int NB = 4;
@@ -93,7 +98,7 @@ __global__ void __launch_bounds__(THREADS) conf_partial_kernel(const float *__re
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int w = 1; w < THREADS / 32; ++w) combine(m, s, red[w].x, red[w].y);
-        part[(size_t)row * gridDim.x + sx] = make_float2(m, s);
+        part[(size_t)row * splits + sx] = make_float2(m, s);
     }
 }
 
@@ -167,8 +172,10 @@ extern "C" int spork_confidence(spork_ctx *c, int n_spans, const int32_t *span_i
     const int32_t *d_span = (const int32_t *)c->conf_desc.p;
     const int32_t *d_rows = (const int32_t *)((const char *)c->conf_desc.p + ib);
     if (n_rows > 0) {
-        conf_partial_kernel<<<dim3(splits, n_rows), THREADS, 0, st>>>(logits, vocab, chunk, d_rows,
-                                                                      (float2 *)c->ws_conf.p);
+        if ((int64_t)splits * n_rows > INT_MAX) return SPORK_ERR_INVALID;
+        const int vec = (vocab & 3) == 0 && ((uintptr_t)logits & 15) == 0;   // else scalar loads (e.g. a sliced tensor)
+        conf_partial_kernel<<<(unsigned)(splits * n_rows), THREADS, 0, st>>>(logits, vocab, chunk, splits, vec, d_rows,
+                                                                             (float2 *)c->ws_conf.p);
         c->last_launches++;
     }
     conf_span_kernel<<<ceil_div(n_spans, 4), 128, 0, st>>>(d_span, n_spans, (const float2 *)c->ws_conf.p, splits,

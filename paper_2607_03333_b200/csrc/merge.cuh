@@ -1,6 +1,8 @@
 // libspork: LSE-weighted combination of one (q row, q head)'s partials by one warp.
 //   M = max lse_s, w_s = exp(lse_s - M), out = sum w_s o_s / sum w_s, lse = M + ln sum w_s
 // An empty partial has lse = -inf and weight 0; no partial at all: out = 0, lse = -inf.
+// A row's partials come from up to MAX_ROW_REFS segments (one per cascade level it shares with other
+// members of its fork group, plus its private tail), each cut into `nsplit` pieces.
 // The partials were written by the attention kernel(s) just before and sit in L2: every
 // partial is read once, with ld.global.cg.
 #pragma once
@@ -17,35 +19,61 @@ __device__ __forceinline__ float merge_warp_max(float v) {
     return v;
 }
 
-// Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
-// every load of a batch in flight before the first use (pure L2 latency otherwise).
-// The two streams a row draws its partials from (none: nsplit = 0).
-struct RowStreams {
-    StreamDesc pre, suf;
+// The splits of one row, flattened over its refs.  Lane i < nref holds ref i: the partial row of its
+// split 0 (for GQA head j of the row's kv head), its number of splits and their stride.
+struct RowSplits {
+    int base, nsplit, stride, cum_end;   // per lane (ref `lane`)
+    int nref, total;                     // warp-uniform
 };
-__device__ __forceinline__ RowStreams load_row_streams(const StreamDesc *__restrict__ streams, const QRowDesc &d,
-                                                       int kvh) {
-    RowStreams r{{0, 0, 0, 0}, {0, 0, 0, 0}};
-    if (d.pre_stream >= 0) r.pre = streams[d.pre_stream + kvh];
-    if (d.suf_stream >= 0) r.suf = streams[d.suf_stream + kvh];
+__device__ __forceinline__ RowSplits load_row_splits(const QRowDesc &d, const RowRef *__restrict__ refs,
+                                                     const StreamDesc *__restrict__ streams, int kvh, int lane) {
+    RowSplits r;
+    r.nref = d.nref;
+    r.base = 0;
+    r.nsplit = 0;
+    r.stride = 0;
+    if (lane < d.nref) {
+        const RowRef ref = refs[d.ref0 + lane];
+        const StreamDesc sd = streams[ref.stream + kvh];
+        r.base = sd.part_base + ref.off;       // GQA head 0 of the row
+        r.nsplit = sd.nsplit;
+        r.stride = sd.stride;
+    }
+    int x = r.nsplit;                    // inclusive scan over the (<= 8) refs
+#pragma unroll
+    for (int o = 1; o < MAX_ROW_REFS; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+    }
+    r.cum_end = x;
+    r.total = __shfl_sync(0xffffffffu, x, MAX_ROW_REFS - 1);
     return r;
 }
+// partial row of split s of GQA head j (every lane may ask for a different s; all lanes must call);
+// -1 beyond the end
+__device__ __forceinline__ int split_row(const RowSplits &r, int s, int j) {
+    int row = -1;
+    for (int i = 0; i < r.nref; ++i) {
+        const int ce = __shfl_sync(0xffffffffu, r.cum_end, i), ns = __shfl_sync(0xffffffffu, r.nsplit, i);
+        const int b = __shfl_sync(0xffffffffu, r.base, i), st = __shfl_sync(0xffffffffu, r.stride, i);
+        if (s >= ce - ns && s < ce) row = b + (s - (ce - ns)) * st + j;
+    }
+    return row;
+}
 
+// Lane s owns the weight of split s; the partial rows are fetched 8 splits at a time with
+// every load of a batch in flight before the first use (pure L2 latency otherwise).
 template <int NI>   // float4 per lane per row: 1 for D <= 128, 2 for D <= 256
-__device__ __forceinline__ void merge_row(const RowStreams &rs, const QRowDesc &d, int j, int D,
-                                          const float *ws_o, const float *ws_lse, float *out_row,
-                                          float *lse_out, int lane) {
-    const StreamDesc &pre = rs.pre, &suf = rs.suf;
-    const int pre0 = pre.part_base + d.pre_off + j;
-    const int suf0 = suf.part_base + d.suf_off + j;
-    const int n = pre.nsplit + suf.nsplit;
-    auto part = [&](int s) -> size_t {
-        return s < pre.nsplit ? (size_t)pre0 + (size_t)s * pre.stride
-                              : (size_t)suf0 + (size_t)(s - pre.nsplit) * suf.stride;
-    };
-    const float lse_mine = lane < n ? __ldcg(ws_lse + part(lane)) : -INFINITY;   // split `lane`
-    float M = lse_mine;
-    for (int s = lane + 32; s < n; s += 32) M = fmaxf(M, __ldcg(ws_lse + part(s)));
+__device__ __forceinline__ void merge_row(const RowSplits &rs, int j, int D, const float *ws_o, const float *ws_lse,
+                                          float *out_row, float *lse_out, int lane) {
+    const int n = rs.total;
+    const int row_first = split_row(rs, lane, j);                 // split `lane`
+    const float lse_first = row_first >= 0 ? __ldcg(ws_lse + row_first) : -INFINITY;
+    float M = lse_first;
+    for (int s0 = 32; s0 < n; s0 += 32) {
+        const int row = split_row(rs, s0 + lane, j);
+        if (row >= 0) M = fmaxf(M, __ldcg(ws_lse + row));
+    }
     M = merge_warp_max(M);
     const int nv = D >> 2;                        // float4 per row (<= 64)
     float4 *o = reinterpret_cast<float4 *>(out_row);
@@ -60,23 +88,23 @@ __device__ __forceinline__ void merge_row(const RowStreams &rs, const QRowDesc &
     float W = 0.f;
     for (int s0 = 0; s0 < n; s0 += 32) {
         const int nb = min(32, n - s0);
-        const float wl = lane < nb ? expf((s0 == 0 ? lse_mine : __ldcg(ws_lse + part(s0 + lane))) - M)
-                                   : 0.f;                                   // weight of split s0+lane
+        const int row_l = s0 == 0 ? row_first : split_row(rs, s0 + lane, j);
+        const float wl = row_l >= 0 ? expf((s0 == 0 ? lse_first : __ldcg(ws_lse + row_l)) - M) : 0.f;
         for (int b0 = 0; b0 < nb; b0 += 8) {
             float4 v[NI][8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-                const bool have = b0 + u < nb;          // no load beyond the last split
-                const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(have ? s0 + b0 + u : 0) * D);
+                const int row = __shfl_sync(0xffffffffu, row_l, (b0 + u) & 31);   // -1 beyond the last split
+                const float4 *po = reinterpret_cast<const float4 *>(ws_o + (size_t)max(row, 0) * D);
 #pragma unroll
                 for (int i = 0; i < NI; ++i) {
                     const int c = lane + 32 * i;
-                    v[i][u] = have && c < nv ? __ldcg(po + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+                    v[i][u] = (row >= 0 && b0 + u < nb && c < nv) ? __ldcg(po + c) : make_float4(0.f, 0.f, 0.f, 0.f);
                 }
             }
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-                const float ws = __shfl_sync(0xffffffffu, wl, (b0 + u) & 31);   // 0 beyond nb
+                const float ws = b0 + u < nb ? __shfl_sync(0xffffffffu, wl, (b0 + u) & 31) : 0.f;
                 W += ws;
 #pragma unroll
                 for (int i = 0; i < NI; ++i) {
@@ -97,28 +125,23 @@ __device__ __forceinline__ void merge_row(const RowStreams &rs, const QRowDesc &
     if (lane == 0) *lse_out = M + logf(W);
 }
 
-
 // The same combine for JB consecutive GQA heads of one (q row, kv head) at once -- their partial rows
 // are contiguous (JB x D floats per split), so one warp streams JB * 512 B per split with every load
 // of a split in flight: one descriptor fetch and JB times the memory-level parallelism per warp.
 // JB is a power of two <= 8; lane `e` of a batch owns the weight of (split e / JB, head e % JB).
+// The JB heads start at GQA head j0.
 template <int NI, int JB>
-__device__ __forceinline__ void merge_heads(const RowStreams &rs, const QRowDesc &d, int j0, int D,
-                                            const float *ws_o, const float *ws_lse, float *out_rows,
-                                            float *lse_out, int lane) {
-    const StreamDesc &pre = rs.pre, &suf = rs.suf;
-    const int pre0 = pre.part_base + d.pre_off + j0;
-    const int suf0 = suf.part_base + d.suf_off + j0;
-    const int n = pre.nsplit + suf.nsplit;
-    auto part = [&](int s) -> size_t {          // partial row of (split s, head j0)
-        return s < pre.nsplit ? (size_t)pre0 + (size_t)s * pre.stride
-                              : (size_t)suf0 + (size_t)(s - pre.nsplit) * suf.stride;
-    };
+__device__ __forceinline__ void merge_heads(const RowSplits &rs, int j0, int D, const float *ws_o, const float *ws_lse,
+                                            float *out_rows, float *lse_out, int lane) {
+    const int n = rs.total;
     constexpr int SB = 32 / JB;                 // splits per batch of 32 lanes
     const int jj = lane % JB, sl = lane / JB;
     // ---- row maxima ----
     float M = -INFINITY;
-    for (int s = sl; s < n; s += SB) M = fmaxf(M, __ldcg(ws_lse + part(s) + jj));
+    for (int s0 = 0; s0 < n; s0 += SB) {
+        const int row = split_row(rs, s0 + sl, j0);
+        if (row >= 0) M = fmaxf(M, __ldcg(ws_lse + row + jj));
+    }
 #pragma unroll
     for (int o = JB; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));   // lanes of head jj
     const int nv = D >> 2;
@@ -131,11 +154,12 @@ __device__ __forceinline__ void merge_heads(const RowStreams &rs, const QRowDesc
         for (int i = 0; i < NI; ++i) acc[k][i] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     for (int s0 = 0; s0 < n; s0 += SB) {
-        const int s_mine = s0 + sl;
-        const float wl = (s_mine < n && M != -INFINITY) ? expf(__ldcg(ws_lse + part(s_mine) + jj) - M) : 0.f;
+        const int row_l = split_row(rs, s0 + sl, j0);        // head j0's partial row of split s0 + sl
+        const float wl = (row_l >= 0 && M != -INFINITY) ? expf(__ldcg(ws_lse + row_l + jj) - M) : 0.f;
         const int nb = min(SB, n - s0);
         for (int sb = 0; sb < nb; ++sb) {
-            const float4 *po = reinterpret_cast<const float4 *>(ws_o + part(s0 + sb) * D);
+            const int row = __shfl_sync(0xffffffffu, row_l, sb * JB);
+            const float4 *po = reinterpret_cast<const float4 *>(ws_o + (size_t)row * D);
             float4 v[JB][NI];
 #pragma unroll
             for (int k = 0; k < JB; ++k)

@@ -17,9 +17,13 @@ constexpr int PS = SPORK_PAGE_SIZE;  // tokens per page
 // ---------------------------------------------------------------------------
 // One item = one (segment, split, kv head, row block): `nrows` query rows
 // against tokens [tok0, tok1) of the sequence in slot `table_seq`.
-// Logical row r (rb0 <= r < rb0 + nrows) is q row (qrow0 + r / G), q head
-// (kvh * G + r % G).  Token t is visible to row r iff t <= lim0 + r / G
-// (lim0 = INT_MAX/2 for shared-prefix items: no mask).
+// Logical row r (rb0 <= r < rb0 + nrows) is q head (kvh * G + r % G) of the segment's (r / G)-th
+// q row: q row qrow0 + r / G, or rowmap[rowmap + r / G] when the segment's rows are not
+// consecutive in the call (a sub-tree of a fork group).  Token t is visible to row r iff
+// t <= lim0 + r / G (lim0 = INT_MAX/2 for shared segments: no mask).
+// Items of a private tail carry flags: ITEM_LEN_LIM: lim0 = len[table_seq] - lim_k, and on the
+// tail's last piece ITEM_LEN_TOK1: tok1 = len[table_seq], both read from the DEVICE lengths when the
+// kernel runs -- a plan stays valid while its sequences grow by appended tokens.
 struct WorkItem {
     int32_t table_seq;
     int32_t tok0;       // multiple of 16
@@ -30,9 +34,12 @@ struct WorkItem {
     int32_t nrows;      // <= 64 (mma.sync / simt path), <= 128 / 256 (tcgen05 kernel, one / two pipes)
     int32_t lim0;
     int32_t part_base;  // partial row index of logical row rb0
-    int32_t pad[3];
+    int32_t flags;      // ITEM_*
+    int32_t lim_k;
+    int32_t rowmap;     // -1: rows are consecutive from qrow0
 };
 static_assert(sizeof(WorkItem) == 48, "WorkItem layout");
+enum : int32_t { ITEM_LEN_LIM = 1, ITEM_LEN_TOK1 = 2 };
 
 // A stream = (segment, kv head): the partials of its rows.  Partial row index of
 // (split s, row i of the stream) = part_base + s * stride + i, rows ordered (q row, GQA head).
@@ -42,12 +49,31 @@ struct StreamDesc {
 };
 static_assert(sizeof(StreamDesc) == 16, "StreamDesc layout");
 
-// Per q row: its shared-prefix stream and its private stream of kv head 0 (-1: none; kv head h
-// is stream + h) and the row's offset q_index * G inside them.
-struct QRowDesc {
-    int32_t pre_stream, pre_off, suf_stream, suf_off;
+// Per q row: the segments it has partials in -- one per cascade level it shares with other members
+// of its fork group, plus its private tail: refs [ref0, ref0 + nref).  A ref names the segment's
+// stream of kv head 0 (kv head h is stream + h) and the row's offset (q index in the segment) * G.
+struct RowRef {
+    int32_t stream, off;
 };
-static_assert(sizeof(QRowDesc) == 16, "QRowDesc layout");
+struct QRowDesc {
+    int32_t ref0, nref;
+};
+static_assert(sizeof(QRowDesc) == 8 && sizeof(RowRef) == 8, "merge descriptor layout");
+constexpr int MAX_ROW_REFS = 8;     // deepest cascade: 7 shared levels + the private tail
+
+// Host lineage of a sequence: which incarnation allocated each of its pages, run-length encoded.
+// Pages [r[i-1].end, r[i].end) were allocated by incarnation r[i].uid (a fresh uid is drawn at
+// seq_create, at fork (for the child) and at truncate).  Two sequences hold the same physical page at
+// index j exactly when their labels at j are equal, so the common leading pages of any set of
+// sequences follow from the host alone (no device read-back).  More than MAX_RUNS runs: the deepest
+// ones are folded into a private run, which can only under-state sharing.
+struct Lineage {
+    static constexpr int MAX_RUNS = 8;
+    int32_t n = 0;
+    int32_t end[MAX_RUNS];
+    uint64_t uid[MAX_RUNS];
+    int pages() const { return n ? end[n - 1] : 0; }
+};
 
 // ---------------------------------------------------------------------------
 // staging ring: pinned host + device scratch for per-call descriptors
@@ -71,17 +97,22 @@ struct Plan {
     uint64_t structure_epoch = 0, len_epoch = 0;
     bool verify = false;
     std::vector<int32_t> group_indptr, seq_ids, q_indptr;
-    std::vector<int32_t> shared_pages;  // per group (level-1 cache)
-    bool shared_valid = false;
-    uint64_t shared_epoch = 0;
-    std::vector<int32_t> shared_key_indptr, shared_key_ids;
-    // device copies
-    DevBuf items, qdesc, streams;
-    // items = [n_items of the mma.sync / simt path][n_items_umma of the tcgen05 kernel, <= 128 rows]
-    //         [n_items_umma2 of the two-pipe tcgen05 kernel, <= 256 rows];
-    // cta_ptr = int32[grid + 1], int32[grid_umma + 1], int32[grid_umma2 + 1]: CTA b of a kernel
-    // runs items [cta_ptr[b], cta_ptr[b + 1]) of its own list
-    DevBuf cta_ptr;
+    std::vector<int32_t> base_len;   // lengths the plan was built for; it stays valid while
+                                     // base_len <= len < base_len + GROW_WINDOW for every sequence
+    bool growable = false;
+    int64_t base_unique = 0, base_naive = 0;
+    // device copy: ONE buffer
+    //   items   = [n_items of the mma.sync / simt path][n_items_umma of the tcgen05 kernel, <= 128 rows]
+    //             [n_items_umma2 of the two-pipe tcgen05 kernel, <= 256 rows]
+    //   cta_ptr = int32[grid + 1], int32[grid_umma + 1], int32[grid_umma2 + 1]: CTA b of a kernel
+    //             runs items [cta_ptr[b], cta_ptr[b + 1]) of its own list
+    DevBuf blob;
+    const WorkItem *d_items = nullptr;
+    const QRowDesc *d_qdesc = nullptr;
+    const RowRef *d_refs = nullptr;
+    const StreamDesc *d_streams = nullptr;
+    const int32_t *d_cta_ptr = nullptr;
+    const int32_t *d_rowmap = nullptr;
     int n_items = 0, n_qrows = 0, grid = 0;
     int n_items_umma = 0, grid_umma = 0;
     int n_items_umma2 = 0, grid_umma2 = 0;
@@ -119,6 +150,9 @@ struct spork_ctx {
     std::vector<int32_t> h_fork_nf;      // full pages it shared with its parent at that fork
     uint64_t fork_calls = 0;
     std::vector<int32_t> h_scratch;      // per-slot scratch (fork counts, evolving lens)
+    std::vector<spork::Lineage> h_lin;   // page lineage per slot (see Lineage)
+    std::vector<uint64_t> h_uid;         // current incarnation of the slot
+    uint64_t next_uid = 1;
     int64_t free_lb;                     // lower bound on free pages
     int n_live;
 
@@ -135,12 +169,15 @@ struct spork_ctx {
     std::vector<int32_t> conf_key;
     void *h_io = nullptr;         // pinned bounce (unused if caller memory is pinned)
     int last_launches;
-    cudaEvent_t plan_ev;
-    bool plan_ev_pending;
+    int plan_builds = 0;
+    uint32_t smem_attr_done = 0;          // bit per kernel: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) done on this device
     int timing = 0;
     int stream_k = 1;             // equal-work contiguous schedule when every segment is one row block
     int many_row_variant = 0;             // segments of > 128 rows: 0 default kernel, 1 two-pipe, 2 split-row kernel
     int umma_min_rows = 1;        // segments with at least this many rows take the tcgen05 path
+    int cascade_levels = spork::MAX_ROW_REFS - 1;   // deepest cascade the planner builds (1: the group-wide prefix only)
+    std::vector<void *> layer_k, layer_v;   // pools of layers 1.. (layer 0 = k_pool / v_pool), see spork_layers
+    spork::DevBuf d_layer_pools;            // the same pointers on the device: k of layers 1.., then v of layers 1..
     cudaEvent_t t_ev[3] = {nullptr, nullptr, nullptr};
     bool t_valid = false;
 };
@@ -170,13 +207,25 @@ int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st);  // OOM check (ma
 int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
                const int32_t *q_indptr, cudaStream_t st);
 
-// attention launchers
-int launch_attn_simt(spork_ctx *c, const void *q, cudaStream_t st);
-int launch_merge(spork_ctx *c, float *out, float *lse, cudaStream_t st);
+// lineage (alloc.cu keeps it up to date, plan.cu reads it)
+void lineage_reset(spork_ctx *c, int s);                       // seq_create / release
+void lineage_grow(spork_ctx *c, int s, int n_pages);           // append: pages [old, n_pages) are the slot's own
+void lineage_fork(spork_ctx *c, int child, int parent, int len);
+void lineage_truncate(spork_ctx *c, int s, int keep_pages);
+int lineage_lcp(const Lineage &a, const Lineage &b);           // common leading pages
+uint64_t lineage_label(const Lineage &a, int page);            // 0: no such page
+
+// attention launchers: one layer = (K pool, V pool, q, out, lse)
+struct LayerIO {
+    const void *k_pool, *v_pool, *q;
+    float *out, *lse;
+};
+int launch_attn_simt(spork_ctx *c, const LayerIO &io, cudaStream_t st);
+int launch_merge(spork_ctx *c, const LayerIO &io, cudaStream_t st);
 int attn_mma_grid(spork_ctx *c);
-int launch_attn_umma(spork_ctx *c, const void *q, int np, bool programmatic, cudaStream_t st);
+int launch_attn_umma(spork_ctx *c, const LayerIO &io, int np, bool programmatic, bool wait_prev, cudaStream_t st);
 int attn_umma_grid(spork_ctx *c, int variant);
-int launch_attn_mma(spork_ctx *c, const void *q, bool programmatic, cudaStream_t st);
+int launch_attn_mma(spork_ctx *c, const LayerIO &io, bool programmatic, cudaStream_t st);
 
 // Swizzled (page, kv head) block, bf16 with D % 64 == 0: the block is a run of 1 KiB
 // atoms of 8 token rows x 128 bytes (64 dims), ordered [row group r/8][dim half d/64];
@@ -193,5 +242,23 @@ __host__ __device__ inline int head_block_off(int swizzled, int D, int r, int d)
     if (!swizzled) return r * D + d;
     return (swz_chunk_off(D >> 6, r, d >> 3) >> 1) + (d & 7);
 }
+
+#ifdef __CUDACC__
+// The item as the kernel runs it: lengths that the plan left open are read from the device now.
+__device__ __forceinline__ WorkItem load_item(const WorkItem *__restrict__ items, int idx,
+                                              const int32_t *__restrict__ len) {
+    WorkItem it = items[idx];
+    if (it.flags) {
+        const int L = len[it.table_seq];
+        if (it.flags & ITEM_LEN_TOK1) it.tok1 = L;
+        if (it.flags & ITEM_LEN_LIM) it.lim0 = L - it.lim_k;
+    }
+    return it;
+}
+// q row of logical row lr of the item
+__device__ __forceinline__ int item_qrow(const WorkItem &it, const int32_t *__restrict__ rowmap, int lr, int G) {
+    return it.rowmap < 0 ? it.qrow0 + lr / G : rowmap[it.rowmap + lr / G];
+}
+#endif
 
 }  // namespace spork

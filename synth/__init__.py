@@ -36,6 +36,8 @@ T_OUTLIER_PREFIX = 6
 T_OUTLIER_SUFFIX = 7
 T_CHURN = 8
 T_MISC = 9
+T_COT_K = 10
+T_COT_V = 11
 
 
 def rng(cfg_no: int, tensor_no: int, index: int = 0) -> np.random.Generator:
@@ -256,7 +258,7 @@ class Workload:
 # ----------------------------------------------------------------------------
 # the call script (same calls, same order, for every engine)
 # ----------------------------------------------------------------------------
-def build_state(engine, wl: Workload, interleave: bool = True) -> np.ndarray:
+def build_state(engine, wl: Workload, interleave: bool = True, values: bool = True) -> np.ndarray:
     """Replays SURVEY.md 8(d) "Placement" through an engine exposing
     seq_create(n)->ids, append(seq_ids, n_tokens, k, v), fork(parents)->children.
 
@@ -265,11 +267,14 @@ def build_state(engine, wl: Workload, interleave: bool = True) -> np.ndarray:
     tokens are appended round-robin one page at a time across all sequences so
     that private pages interleave as under continuous batching.
     Returns seq_ids[n_seqs] in workload order (main first within each group).
+    values=False replays the same calls with all-zero K/V (for engines whose allocator is all that
+    matters, e.g. the fork-churn baseline): block tables and refcounts are the same.
     """
     c = wl.cfg
     mains = np.asarray(engine.seq_create(c.n_groups), dtype=np.int32)
+    zeros = None if values else np.zeros((max(c.prefix_len, 1), c.Hkv, c.D), storage_np_dtype(c.dtype))
     for g in range(c.n_groups):
-        pk, pv = wl.prefix_kv(g)
+        pk, pv = wl.prefix_kv(g) if values else (zeros[:c.prefix_len], zeros[:c.prefix_len])
         engine.append(mains[g:g + 1], np.array([c.prefix_len], np.int32), pk, pv)
     seq_ids = np.zeros(c.n_seqs, dtype=np.int32)
     n_probe = c.group_size - 1
@@ -281,7 +286,7 @@ def build_state(engine, wl: Workload, interleave: bool = True) -> np.ndarray:
         for j in range(n_probe):
             seq_ids[g * c.group_size + 1 + j] = children[g * n_probe + j]
 
-    priv = [wl.suffix_kv(i) for i in range(c.n_seqs)]
+    priv = [wl.suffix_kv(i) for i in range(c.n_seqs)] if values else None
     done = np.zeros(c.n_seqs, dtype=np.int64)
     step = c.page_size if interleave else int(max(1, wl.private_len.max()))
     while True:
@@ -289,6 +294,91 @@ def build_state(engine, wl: Workload, interleave: bool = True) -> np.ndarray:
         if todo.size == 0:
             break
         n_tok = np.minimum(step, wl.private_len[todo] - done[todo]).astype(np.int32)
+        if values:
+            ks = np.concatenate([priv[i][0][done[i]:done[i] + n] for i, n in zip(todo, n_tok)], axis=0)
+            vs = np.concatenate([priv[i][1][done[i]:done[i] + n] for i, n in zip(todo, n_tok)], axis=0)
+        else:
+            ks = vs = np.zeros((int(n_tok.sum()), c.Hkv, c.D), storage_np_dtype(c.dtype))
+        engine.append(seq_ids[todo], n_tok, ks, vs)
+        done[todo] += n_tok
+    return seq_ids
+
+
+# ----------------------------------------------------------------------------
+# successive probes (Algorithm 1 steps 4-6; Fig. 4)
+# ----------------------------------------------------------------------------
+class SuccessiveWorkload(Workload):
+    """Probe r (r = 1 .. group_size-1) of a group is forked after the main stream has decoded
+    r * stride further CoT tokens, so it shares P + r * stride tokens with the main stream (and with
+    every later probe), not just P.  Token content per group: prefix(g), then the group's CoT stream
+    cot(g) of (group_size-1) * stride tokens (the main stream's tokens between the fork points), then
+    each sequence's private tokens (suffix, then drafts) from its own sub-stream."""
+
+    def __init__(self, cfg: SporkConfig, stride: int, k_per_seq: Optional[Sequence[int]] = None):
+        super().__init__(cfg, k_per_seq)
+        self.stride = int(stride)
+        gs = cfg.group_size
+        r = np.arange(cfg.n_seqs) % gs                       # 0: main, r: probe r
+        self.fork_extra = np.where(r == 0, (gs - 1) * self.stride, r * self.stride).astype(np.int64)
+        self.total_len = cfg.prefix_len + self.fork_extra + self.private_len
+
+    def cot_kv(self, g: int):
+        c = self.cfg
+        n = (c.group_size - 1) * self.stride
+        k = self._outliers(self._normal(T_COT_K, g, n, c.Hkv), T_OUTLIER_PREFIX, 1_000_000 + g)
+        v = self._normal(T_COT_V, g, n, c.Hkv)
+        return to_storage(k, c.dtype), to_storage(v, c.dtype)
+
+    def unique_tokens(self) -> int:
+        """Nested sharing: every token is counted once per group.  A fork point that is not page
+        aligned duplicates its partially filled page into the probe (those tokens are private copies)."""
+        c = self.cfg
+        dup = sum((c.prefix_len + r * self.stride) % c.page_size for r in range(1, c.group_size))
+        return int(c.n_groups * (c.prefix_len + (c.group_size - 1) * self.stride + dup) + self.private_len.sum())
+
+    def single_level_tokens(self) -> int:
+        """What a cascade with ONE shared level reads: the group-wide common prefix (up to the first
+        fork point) once, everything beyond it once per member."""
+        c = self.cfg
+        if c.group_size < 2:
+            return self.naive_tokens()
+        shared = ((c.prefix_len + self.stride) // c.page_size) * c.page_size
+        return int(c.n_groups * shared + (self.total_len - shared).sum())
+
+    def dense_kv(self, seq: int):
+        g = self.group_of(seq)
+        pk, pv = self.prefix_kv(g)
+        ck, cv = self.cot_kv(g)
+        sk, sv = self.suffix_kv(seq)
+        e = int(self.fork_extra[seq])
+        return np.concatenate([pk, ck[:e], sk], axis=0), np.concatenate([pv, cv[:e], sv], axis=0)
+
+
+def build_state_successive(engine, wl: SuccessiveWorkload) -> np.ndarray:
+    """The call script of one paper turn per group (Algorithm 1): main prefilled,
+    then for r = 1 .. R: main decodes `stride` more CoT tokens (step 5), probe r is forked from it
+    (step 6); afterwards every stream appends its private tokens round-robin one page at a time."""
+    c = wl.cfg
+    mains = np.asarray(engine.seq_create(c.n_groups), dtype=np.int32)
+    for g in range(c.n_groups):
+        pk, pv = wl.prefix_kv(g)
+        engine.append(mains[g:g + 1], np.array([c.prefix_len], np.int32), pk, pv)
+    seq_ids = np.zeros(c.n_seqs, dtype=np.int32)
+    seq_ids[0::c.group_size] = mains
+    cot = [wl.cot_kv(g) for g in range(c.n_groups)]
+    st = wl.stride
+    for r in range(1, c.group_size):
+        ks = np.concatenate([cot[g][0][(r - 1) * st:r * st] for g in range(c.n_groups)], axis=0)
+        vs = np.concatenate([cot[g][1][(r - 1) * st:r * st] for g in range(c.n_groups)], axis=0)
+        engine.append(mains, np.full(c.n_groups, st, np.int32), ks, vs)
+        seq_ids[r::c.group_size] = np.asarray(engine.fork(mains), dtype=np.int32)
+    priv = [wl.suffix_kv(i) for i in range(c.n_seqs)]
+    done = np.zeros(c.n_seqs, dtype=np.int64)
+    while True:
+        todo = np.nonzero(done < wl.private_len)[0]
+        if todo.size == 0:
+            break
+        n_tok = np.minimum(c.page_size, wl.private_len[todo] - done[todo]).astype(np.int32)
         ks = np.concatenate([priv[i][0][done[i]:done[i] + n] for i, n in zip(todo, n_tok)], axis=0)
         vs = np.concatenate([priv[i][1][done[i]:done[i] + n] for i, n in zip(todo, n_tok)], axis=0)
         engine.append(seq_ids[todo], n_tok, ks, vs)

@@ -35,6 +35,36 @@ def pool_dims(wl: synth.Workload, slack_pages: int = 64):
     return total, c.n_seqs + 8, per_seq
 
 
+class Both:
+    """synth.build_state engine that replays every call on the oracle AND on libspork (the generated
+    K/V values are produced once), checking that both hand out the same ids."""
+
+    def __init__(self, orc, spk):
+        self.orc, self.spk = orc, spk
+
+    def seq_create(self, n):
+        a, b = self.orc.seq_create(n), self.spk.seq_create(n)
+        assert np.array_equal(a, b)
+        return a
+
+    def append(self, seq_ids, n_tokens, k, v):
+        self.orc.append(seq_ids, n_tokens, k, v)
+        self.spk.append(seq_ids, n_tokens, k, v)
+
+    def fork(self, parents):
+        a, b = self.orc.fork(parents), self.spk.fork(parents)
+        assert np.array_equal(a, b)
+        return a
+
+    def release(self, seq_ids):
+        self.orc.release(seq_ids)
+        self.spk.release(seq_ids)
+
+    def truncate(self, seq_ids, new_len):
+        self.orc.truncate(seq_ids, new_len)
+        self.spk.truncate(seq_ids, new_len)
+
+
 def assert_state_equal(orc, spk, seq_ids, check_kv_tail=True):
     """bit-exact lengths, block tables and refcounts (device vs oracle)."""
     for s in seq_ids:
