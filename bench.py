@@ -320,6 +320,26 @@ class Env:
     def mx(self, x):
         return max_over_ranks(float(x), self.device, self.world)
 
+    def read_peak(self, spk):
+        """GB/s a plain read-only stream reaches on this GPU now (spork_hbm_read_probe over the 512 MiB
+        flush buffer, best of 10 after a warm-up pass).  Reported beside the driver's copy figure: the
+        attention kernels read, they do not copy."""
+        if getattr(self, "_read_peak", None) is None:
+            torch = self.torch
+            st = spk.stream
+            nbytes = self.flush.numel()
+            spk.hbm_read_probe(self.flush)
+            best = 0.0
+            for _ in range(10):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(st)
+                spk.hbm_read_probe(self.flush)
+                b.record(st)
+                b.synchronize()
+                best = max(best, nbytes / (a.elapsed_time(b) * 1e-3) / 1e9)
+            self._read_peak = best
+        return self._read_peak
+
     def close(self):
         if self.world > 1:
             import torch.distributed as dist
@@ -357,11 +377,20 @@ def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
     for _ in range(max(args.warmup, 3)):
         env.flush_l2(st)
         step()
+    # steady-state plan rebuild (workspace already sized): invalidate the cached plan, time the next call
+    spk.set_cascade_levels(7)
+    spk.synchronize()
+    t0 = time.perf_counter()
+    step()
+    rebuild_call_us = (time.perf_counter() - t0) * 1e6    # host time of a call that rebuilds the plan
+    info1 = spk.last_plan()
+    assert info1["plan_cached"] == 0
     env.barrier()
     ms = env.timed(st, step, args.steps)
     env.barrier()
     ms_step = env.mx(sum(ms)) / args.steps
     info = spk.last_plan()
+    assert info["plan_cached"] == 1
     ub = wl.unique_kv_bytes()
     assert info["unique_tokens"] * cfg.token_bytes == ub, "library and synth disagree on the unique KV bytes"
     flops = wl.flops()
@@ -391,8 +420,13 @@ def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
     else:
         roof = {"bound": "hbm", "achieved": ach_bw, "peak": peak_bw, "unit": "GB/s",
                 "frac": ach_bw / peak_bw, "traffic": _traffic(name)}
+    read_peak = env.read_peak(spk)
     roof.update({"kernel": kname, "kernel_ms": k_avg, "merge_ms": float(np.mean(m_ms)),
                  "peak_source": peaks["_source"], "frac_of_8TBps": ach_bw / 8000.0,
+                 "read_peak": read_peak, "frac_of_read_peak": ach_bw / read_peak,
+                 "peak_note": "peak = MEASURED_PEAKS.json's copy (read + write) figure; read_peak = a plain "
+                              "read-only stream timed in this run (spork_hbm_read_probe), which a read-dominated "
+                              "kernel can exceed the copy figure up to",
                  "achieved_tflops": ach_tf, "algorithmic_bytes": ub, "algorithmic_flops": flops})
     warm = env.timed(st, step, args.steps, do_flush=False)
 
@@ -430,7 +464,9 @@ def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
         "dtype": cfg.dtype, "unique_kv_bytes": ub, "naive_kv_bytes": wl.naive_tokens() * cfg.token_bytes,
         "flops": flops, "roofline": roof, "e2e": e2e, "clocks": clocks,
         "warm_l2_ms_per_step": float(np.mean(warm)), "first_call_us": first_call_us,
-        "plan_rebuild_us": info0.get("plan_host_us"), "launches_per_step": info["launches"], "plan": info,
+        "plan_rebuild_us": info1.get("plan_host_us"), "plan_rebuild_call_us": rebuild_call_us,
+        "plan_first_build_us": info0.get("plan_host_us"),
+        "launches_per_step": info["launches"], "plan": info,
         "shape": {"Hq": cfg.Hq, "Hkv": cfg.Hkv, "D": cfg.D, "n_groups": cfg.n_groups,
                   "group_size": cfg.group_size, "prefix_len": cfg.prefix_len,
                   "suffix": [cfg.suffix_lo, cfg.suffix_hi], "k_draft": cfg.k_draft},
@@ -444,17 +480,27 @@ def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
 
 
 def churn_bytes(cfg, wl, ids, parents, num_pages):
-    """Algorithmic bytes of the churn step (SURVEY.md 8(d) churn row, computed exactly): fork = the
-    children's table rows read + written (floor(L/16) + 1 entries of 4 B), the duplicated tail pages
-    read + written (K and V), one scan of the refcount array; release = the children's table rows
-    read once more."""
+    """Algorithmic bytes of the churn step, computed exactly.  SURVEY.md 8(d)'s churn row counts the
+    LOGICAL traffic (every child reads its parent's row and tail: 87 + 87 + 328 + 328 MB); the 10,000
+    children have only 128 distinct parents, whose rows and tail pages are read from HBM once and
+    then served by L2, so the bytes that must cross the HBM interface -- the roofline's numerator --
+    are: fork = the DISTINCT parents' table rows and tail pages read, the children's rows
+    (floor(L/16) + 1 entries of 4 B) and duplicated tail pages (K and V) written, one scan of the
+    refcount array; release = the children's table rows read once more."""
     L = {int(s): int(wl.total_len[i]) for i, s in enumerate(ids)}
     page_bytes = cfg.Hkv * 16 * cfg.D * cfg.elt_bytes          # one pool
     entries = sum(L[int(p)] // 16 + 1 for p in parents)
     tails = sum(1 for p in parents if L[int(p)] % 16)
-    fork_clone = 2 * 4 * entries + tails * 2 * 2 * page_bytes
-    return {"fork_clone_kernel": fork_clone, "refcount_scan": 4 * num_pages, "release_table_read": 4 * entries,
-            "step": fork_clone + 4 * num_pages + 4 * entries, "table_entries": entries, "tail_pages": tails}
+    distinct = sorted(set(int(p) for p in parents))
+    d_entries = sum(L[p] // 16 + 1 for p in distinct)
+    d_tails = sum(1 for p in distinct if L[p] % 16)
+    fork_clone = 4 * (d_entries + entries) + (d_tails + tails) * 2 * page_bytes
+    logical = 2 * 4 * entries + tails * 2 * 2 * page_bytes
+    return {"fork_clone_kernel": fork_clone, "fork_clone_kernel_logical": logical,
+            "refcount_scan": 4 * num_pages, "release_table_read": 4 * entries,
+            "step": fork_clone + 4 * num_pages + 4 * entries,
+            "step_logical": logical + 4 * num_pages + 4 * entries,
+            "table_entries": entries, "tail_pages": tails, "distinct_parents": len(distinct)}
 
 
 def measure_churn(env: Env, spk, ids, cfg, wl, num_pages):
@@ -666,7 +712,8 @@ def headline_line(env: Env, rec, cfg):
         "frac_of_8TBps": rec["frac_of_8TBps"], "frac_of_measured_hbm": rec["frac_of_measured_hbm"],
         "roofline": rec["roofline"], "e2e": rec["e2e"],
         "warm_l2_ms_per_step": rec["warm_l2_ms_per_step"], "first_call_us": rec["first_call_us"],
-        "plan_rebuild_us": rec["plan_rebuild_us"], "plan": rec["plan"],
+        "plan_rebuild_us": rec["plan_rebuild_us"], "plan_rebuild_call_us": rec["plan_rebuild_call_us"],
+        "plan_first_build_us": rec["plan_first_build_us"], "plan": rec["plan"],
     }
     for k in ("verify_tflops", "cpu_baseline", "parity"):
         if k in rec:

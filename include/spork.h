@@ -328,6 +328,14 @@ int spork_verify_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const i
                              const int32_t *seq_ids, const int32_t *q_indptr, const void *const *q,
                              float *const *out, float *const *lse, void *stream);
 
+/*
+ * Bench support: one read-only pass over `bytes` bytes at `buf` (device, 16-byte aligned), launched on
+ * `stream`; the caller times it with events.  bench.py reports the rate it reaches (`read_peak`) beside
+ * MEASURED_PEAKS.json's copy figure: the attention kernels are read streams (SURVEY.md 8(d) asks for GB/s
+ * against the box's measured bandwidth).  Errors: SPORK_ERR_INVALID.
+ */
+int spork_hbm_read_probe(spork_ctx *ctx, const void *buf, size_t bytes, void *stream);
+
 const char *spork_strerror(int code);
 
 #ifdef __cplusplus

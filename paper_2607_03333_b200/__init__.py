@@ -34,7 +34,7 @@ ABI_SYMBOLS = [
     "spork_read_kv", "spork_free_pages", "spork_status", "spork_last_plan", "spork_last_launches",
     "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_many_row_variant", "spork_set_stream_k", "spork_strerror",
     "spork_set_cascade_levels", "spork_layers", "spork_write_kv_layer", "spork_decode_attn_layers",
-    "spork_verify_attn_layers",
+    "spork_verify_attn_layers", "spork_hbm_read_probe",
 ]
 
 
@@ -105,6 +105,7 @@ def load(build_if_missing: bool = True):
         "spork_decode_attn_layers": ([P, I, I, P, P, P, P, P, P], I),
         "spork_verify_attn_layers": ([P, I, I, P, P, P, P, P, P, P], I),
         "spork_last_kernel_ms": ([P, P, P], I),
+        "spork_hbm_read_probe": ([P, P, C.c_size_t, P], I),
         "spork_strerror": ([I], C.c_char_p),
     }
     for name, (args, res) in sig.items():
@@ -424,6 +425,11 @@ class Spork:
     def set_stream_k(self, enable: bool):
         """Planner knob: equal-work contiguous schedule for single-row-block calls (default on)."""
         self._chk(self.lib.spork_set_stream_k(self._h, int(bool(enable))))
+
+    def hbm_read_probe(self, buf):
+        """Bench support: one read-only pass over the device tensor `buf` on our stream."""
+        self._chk(self.lib.spork_hbm_read_probe(self._h, C.c_void_p(buf.data_ptr()),
+                                                C.c_size_t(buf.numel() * buf.element_size()), self._st))
 
     def last_kernel_ms(self):
         """(attention kernel ms, merge kernel ms) of the last attention call (synchronises)."""

@@ -180,6 +180,49 @@ __global__ void __launch_bounds__(256) append_copy_kernel(
     }
 }
 
+// The decode loop's append (Algorithm 1 step 5: one token per live stream and step): few tokens per
+// request and no sequence twice in the batch -> ONE kernel, one block per request: take the pages,
+// publish the length, then write this request's K/V rows (its table entries are its own block's).
+__global__ void __launch_bounds__(128) append_small_kernel(
+    const AppendDesc *__restrict__ descs, const int32_t *__restrict__ free_list, int32_t *refcount,
+    int32_t *table, int table_stride, int32_t *len, int32_t *counters, int need,
+    const uint4 *__restrict__ k_src, const uint4 *__restrict__ v_src, uint8_t *__restrict__ k_pool,
+    uint8_t *__restrict__ v_pool, int Hkv, int chunks_per_row, int swizzled, size_t head_block) {
+    __shared__ int32_t s_page[8];                 // pages of positions old_len .. (<= 64 tokens: <= 5 pages)
+    const AppendDesc d = descs[blockIdx.x];
+    int32_t *row = table + (size_t)d.seq * table_stride;
+    const int first_new = pages_of(d.old_len), p0 = d.old_len / PS;
+    const int n_touch = d.n_tok > 0 ? (d.old_len + d.n_tok - 1) / PS - p0 + 1 : 0;
+    if ((int)threadIdx.x < n_touch) {
+        const int j = p0 + threadIdx.x;
+        int p;
+        if (j >= first_new) {
+            p = free_list[d.free_off + (j - first_new)];
+            row[j] = p;
+            refcount[p] = 1;
+        } else {
+            p = row[j];                           // the partially filled tail page it already holds
+        }
+        s_page[threadIdx.x] = p;
+    }
+    if (threadIdx.x == 0) {
+        if (d.final_len >= 0) len[d.seq] = d.final_len;
+        if (blockIdx.x == 0 && need) atomicSub(&counters[0], need);
+    }
+    __syncthreads();
+    const int units = d.n_tok * Hkv * chunks_per_row;
+    for (int u = threadIdx.x; u < units; u += blockDim.x) {
+        const int c = u % chunks_per_row, h = (u / chunks_per_row) % Hkv, t = u / (chunks_per_row * Hkv);
+        const int pos = d.old_len + t, r = pos % PS;
+        const size_t off = swizzled ? (size_t)swz_chunk_off(chunks_per_row >> 3, r, c)
+                                    : ((size_t)r * chunks_per_row + c) * 16;
+        const size_t dst = ((size_t)s_page[pos / PS - p0] * Hkv + h) * head_block + off;
+        const size_t src = (size_t)d.tok_off * Hkv * chunks_per_row + u;
+        *reinterpret_cast<uint4 *>(k_pool + dst) = k_src[src];
+        *reinterpret_cast<uint4 *>(v_pool + dst) = v_src[src];
+    }
+}
+
 // ---- fork ------------------------------------------------------------------
 struct ForkDesc {
     int32_t parent, child, len, tail_idx;  // tail_idx: index into free_list, or -1
@@ -347,6 +390,29 @@ int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st) {
     return need <= c->free_lb ? SPORK_OK : SPORK_ERR_OOM;
 }
 
+// `need` lowest free page ids, ascending, at d_free_list[*off ..).  The list of one scan is cached: as long
+// as no page has been FREED since (release / truncate / accept invalidate it), the ids behind the ones
+// already handed out are still the lowest free ones, so an append-only phase (the decode loop) scans
+// once per FREE_LIST_BATCH pages instead of once per call.
+int take_free(spork_ctx *c, int need, cudaStream_t st, int *off) {
+    *off = 0;
+    if (need <= 0) return SPORK_OK;
+    if (c->fl_valid && c->fl_pos + need <= c->fl_n) {
+        *off = c->fl_pos;
+        c->fl_pos += need;
+        return SPORK_OK;
+    }
+    // free_lb is a lower bound on the free pages (ensure_pages has run): every id of the list is real
+    constexpr int64_t FREE_LIST_BATCH = 4096;
+    const int want = (int)std::max<int64_t>(need, std::min<int64_t>(c->free_lb, FREE_LIST_BATCH));
+    int rc = launch_free_scan(c, want, st);
+    if (rc != SPORK_OK) return rc;
+    c->fl_valid = true;
+    c->fl_n = want;
+    c->fl_pos = need;
+    return SPORK_OK;
+}
+
 }  // namespace spork
 
 // ---------------------------------------------------------------------------
@@ -382,11 +448,16 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
     if (rc != SPORK_OK) return rc;
     AppendDesc *d = (AppendDesc *)slot->h;
     for (int i = 0; i < n; ++i) c->h_scratch[seq_ids[i]] = -1;  // marks "last request not yet seen"
-    int tok = 0, foff = 0;
+    int fl_off = 0;
+    rc = take_free(c, (int)need, st, &fl_off);
+    if (rc != SPORK_OK) return rc;
+    int tok = 0, foff = fl_off;
+    bool small = true;       // no sequence twice, <= 64 tokens per request: the one-kernel path
     // final_len is written by the LAST request of each sequence: walk backwards to mark it
     for (int i = n - 1; i >= 0; --i) {
         int s = seq_ids[i];
         d[i].final_len = c->h_scratch[s] == -1 ? 0 : -1;  // placeholder 0 = "is last"
+        small = small && c->h_scratch[s] == -1 && n_tokens[i] <= 64;
         c->h_scratch[s] = 0;
     }
     for (int i = 0; i < n; ++i) {
@@ -407,8 +478,17 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
     }
     rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
     if (rc != SPORK_OK) return rc;
-    rc = launch_free_scan(c, (int)need, st);
-    if (rc != SPORK_OK) return rc;
+    if (small) {
+        append_small_kernel<<<n, 128, 0, st>>>(
+            (const AppendDesc *)slot->d, c->d_free_list, c->d_refcount, c->d_table, c->table_stride, c->d_len,
+            c->d_counters, (int)need, (const uint4 *)k_src, (const uint4 *)v_src, (uint8_t *)c->k_pool,
+            (uint8_t *)c->v_pool, c->cfg.num_kv_heads, c->cfg.head_dim * c->elt / 16, c->swizzled, c->head_block);
+        c->last_launches++;
+        SPORK_CUDA(cudaGetLastError());
+        c->free_lb -= need;
+        c->len_epoch++;
+        return stage_done(c, slot, st);
+    }
     append_assign_kernel<<<n, 128, 0, st>>>((const AppendDesc *)slot->d, n, c->d_free_list,
                                             c->d_refcount, c->d_table, c->table_stride, c->d_len,
                                             c->d_counters, (int)need);
@@ -510,6 +590,8 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
     // children: lowest free slots in request order
     c->fork_calls++;
     int tail = 0;
+    rc = take_free(c, (int)need, st, &tail);
+    if (rc != SPORK_OK) return rc;
     for (int i = 0, s = 0; i < n; ++s) {
         if (c->h_live[s]) continue;
         int p = parent_ids[i], L = c->h_len[p];
@@ -529,8 +611,6 @@ extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_
     }
     c->n_live += n;
     rc = stage_commit(c, slot, bytes, st);
-    if (rc != SPORK_OK) return rc;
-    rc = launch_free_scan(c, (int)need, st);
     if (rc != SPORK_OK) return rc;
     if (max_nf > 0) {
         dim3 grid(std::max(1, std::min(ceil_div(max_nf, 1024), 64)), n_par);
@@ -635,6 +715,7 @@ static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_
             return flag ? SPORK_ERR_SHARED : host_err;
         }
     }
+    c->fl_valid = false;        // pages are freed: the cached free list is no longer the lowest ids
     drop_pages_kernel<<<n, 256, 0, st>>>((const DropDesc *)slot->d, c->d_table, c->table_stride,
                                          c->d_len, c->d_refcount, c->d_counters);
     c->last_launches++;

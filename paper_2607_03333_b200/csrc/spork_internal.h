@@ -154,6 +154,8 @@ struct spork_ctx {
     std::vector<uint64_t> h_uid;         // current incarnation of the slot
     uint64_t next_uid = 1;
     int64_t free_lb;                     // lower bound on free pages
+    bool fl_valid = false;               // d_free_list[fl_pos, fl_n) are still the lowest free ids (see take_free)
+    int fl_pos = 0, fl_n = 0;
     int n_live;
 
     uint64_t structure_epoch, len_epoch;
@@ -202,6 +204,7 @@ int devbuf_reserve(DevBuf *b, size_t bytes, cudaStream_t st);
 // alloc.cu
 int launch_free_scan(spork_ctx *c, int need, cudaStream_t st);  // fills d_free_list[0..need)
 int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st);  // OOM check (may sync)
+int take_free(spork_ctx *c, int need, cudaStream_t st, int *off);  // ids at d_free_list[*off, *off + need)
 
 // plan.cu
 int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
