@@ -37,6 +37,19 @@ constexpr int PIPE_COLS = 256;                        // TMEM columns of one pip
 constexpr float LOG2E = 1.4426950408889634f;
 constexpr float LN2 = 0.6931471805599453f;
 constexpr float RESCALE_THRESHOLD = 8.f;              // log2 units
+// share of a tile's exp2 pairs computed on the FMA pipe instead of the MUFU unit (ex2_poly2): pair j of a
+// thread's 32 is emulated when (j * EMU_NUM) % EMU_DEN < EMU_NUM.  Default 0: measured on config 4 the
+// emulation only costs (k = 16: 544 / 568 / 600 / 634 us at 0, 1/4, 1/3, 1/2) -- a softmax warp is bound by
+// its own dependent instruction stream (~2,200 clocks per 64-token tile), not by the
+// MUFU unit, so extra FMA-pipe work lengthens it.  Kept as a build-time knob (-DSPORK_EMU_NUM / _DEN).
+#ifndef SPORK_EMU_NUM
+#define SPORK_EMU_NUM 0
+#endif
+#ifndef SPORK_EMU_DEN
+#define SPORK_EMU_DEN 1
+#endif
+constexpr int EMU_NUM = SPORK_EMU_NUM, EMU_DEN = SPORK_EMU_DEN;
+__host__ __device__ constexpr bool emulated_pair(int j) { return (j * EMU_NUM) % EMU_DEN < EMU_NUM; }
 
 // NP = number of softmax pipes of a CTA = row blocks of 128 it runs against ONE stream of K/V:
 //   NP = 1: items of <= 128 rows, 2 CTAs per SM, 5-slot ring each
@@ -512,7 +525,9 @@ attn_umma_kernel(const UParams P) {
                     float x0, x1, y0, y1;
                     ffma2(x0, x1, __uint_as_float(s0[2 * t]), __uint_as_float(s0[2 * t + 1]), P.scale_log2, nmu);
                     ffma2(y0, y1, __uint_as_float(s1[2 * t]), __uint_as_float(s1[2 * t + 1]), P.scale_log2, nmu);
-                    const float a0 = ex2(x0), a1 = ex2(x1), c0 = ex2(y0), c1 = ex2(y1);
+                    float a0, a1, c0, c1;
+                    if (emulated_pair(2 * t)) ex2_poly2(x0, x1, a0, a1); else { a0 = ex2(x0); a1 = ex2(x1); }
+                    if (emulated_pair(2 * t + 1)) ex2_poly2(y0, y1, c0, c1); else { c0 = ex2(y0); c1 = ex2(y1); }
                     p[t] = pack_bf16(a0, a1);
                     p[16 + t] = pack_bf16(c0, c1);
                     // o is normalised by the sum of the ROUNDED weights the tensor core uses, so that

@@ -185,6 +185,40 @@ __device__ __forceinline__ void fadd2(float &d0, float &d1, float a0, float a1) 
         "mov.b64 {%0, %1}, rd;\n\t}"
         : "+f"(d0), "+f"(d1) : "f"(a0), "f"(a1));
 }
+// 2^x for a PAIR of values on the FMA pipe (the MUFU unit does 16 ex2 per clock and SM, which is what
+// bounds a many-row softmax; a share of the pairs is computed here instead): n = rn(x) by the
+// add-a-big-constant trick, f = x - n in [-0.5, 0.5], 2^f by a degree-4 minimax polynomial (relative
+// error 2.7e-6 in fp32), and n added into the exponent field.  x is clamped to >= -126 (the result is
+// then a denormal-sized number instead of a wrapped exponent; -inf gives ~1e-38, not 0).
+__device__ __forceinline__ void ex2_poly2(float x0, float x1, float &y0, float &y1) {
+    x0 = fmaxf(x0, -126.f);
+    x1 = fmaxf(x1, -126.f);
+    uint32_t r0, r1, p0, p1;
+    asm("{\n\t.reg .b64 x, r, n, f, p, c, m;\n\t"
+        "mov.b64 x, {%4, %5};\n\t"
+        "mov.b64 m, {%6, %6};\n\t"
+        "add.rn.f32x2 r, x, m;\n\t"            // x + 1.5 * 2^23: the integer lands in the low mantissa bits
+        "mov.b64 m, {%7, %7};\n\t"
+        "add.rn.f32x2 n, r, m;\n\t"            // - 1.5 * 2^23: n as a float
+        "mov.b64 m, {%8, %8};\n\t"
+        "fma.rn.f32x2 f, n, m, x;\n\t"         // f = x - n
+        "mov.b64 p, {%9, %9};\n\t"
+        "mov.b64 c, {%10, %10};\n\t"
+        "fma.rn.f32x2 p, p, f, c;\n\t"
+        "mov.b64 c, {%11, %11};\n\t"
+        "fma.rn.f32x2 p, p, f, c;\n\t"
+        "mov.b64 c, {%12, %12};\n\t"
+        "fma.rn.f32x2 p, p, f, c;\n\t"
+        "mov.b64 c, {%13, %13};\n\t"
+        "fma.rn.f32x2 p, p, f, c;\n\t"
+        "mov.b64 {%0, %1}, r;\n\t"
+        "mov.b64 {%2, %3}, p;\n\t}"
+        : "=r"(r0), "=r"(r1), "=r"(p0), "=r"(p1)
+        : "f"(x0), "f"(x1), "f"(12582912.f), "f"(-12582912.f), "f"(-1.f), "f"(0.00957401655614376f),
+          "f"(0.055918190628290176f), "f"(0.2402464896440506f), "f"(0.6931217312812805f), "f"(0.9999992847442627f));
+    y0 = __uint_as_float(p0 + (r0 << 23));
+    y1 = __uint_as_float(p1 + (r1 << 23));
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
     uint32_t r;
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
