@@ -20,8 +20,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "spork_oracle.c")
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-F32, BF16 = 0, 1
-DTYPES = {"f32": F32, "bf16": BF16}
+F32, BF16, E4M3KV = 0, 1, 2
+DTYPES = {"f32": F32, "bf16": BF16, "e4m3": E4M3KV}      # "e4m3": K, V e4m3 bytes, Q bf16
+KV_NP = {"f32": np.float32, "bf16": np.uint16, "e4m3": np.uint8}   # storage arrays are bit patterns
+Q_NP = {"f32": np.float32, "bf16": np.uint16, "e4m3": np.uint16}
 
 OK = 0
 ERR_INVALID, ERR_OOM, ERR_NO_SLOT, ERR_TOO_LONG, ERR_INVALID_SEQ, ERR_SHARED = -1, -2, -3, -4, -5, -6
@@ -63,6 +65,7 @@ def lib():
             "oracle_merge2": ([I, P, D, P, D, P, P], None),
             "oracle_cascade_row": ([P, I, I, P, I, P, P], I),
             "oracle_attend_dense": ([I, I, D, P, P, P, I, P, P], I),
+            "oracle_widen": ([I, P, C.c_long, P], None),
             "oracle_num_threads": ([], I),
         }
         for name, (args, res) in sig.items():
@@ -98,7 +101,8 @@ class Oracle:
         self.dtype, self.Hq, self.Hkv, self.D, self.ps = dtype, Hq, Hkv, D, page_size
         self.num_pages, self.max_seqs, self.max_pages_per_seq = num_pages, max_seqs, max_pages_per_seq
         self.scale = scale
-        self.np_dtype = np.float32 if dtype == "f32" else np.uint16
+        self.np_dtype = KV_NP[dtype]
+        self.q_dtype = Q_NP[dtype]
         self._h = lib().oracle_create(DTYPES[dtype], Hq, Hkv, D, page_size, num_pages, max_seqs,
                                       max_pages_per_seq, float(scale), int(store_kv))
         if not self._h:
@@ -185,7 +189,7 @@ class Oracle:
     # ---- attention ----------------------------------------------------------
     def decode(self, seq_ids, q: np.ndarray):
         s = _i32(seq_ids)
-        q = np.ascontiguousarray(q, dtype=self.np_dtype)
+        q = np.ascontiguousarray(q, dtype=self.q_dtype)
         assert q.shape == (len(s), self.Hq, self.D)
         out = np.zeros((len(s), self.Hq, self.D), np.float64)
         lse = np.zeros((len(s), self.Hq), np.float64)
@@ -194,7 +198,7 @@ class Oracle:
 
     def verify(self, seq_ids, q_indptr, q: np.ndarray, check: bool = True):
         s, qi = _i32(seq_ids), _i32(q_indptr)
-        q = np.ascontiguousarray(q, dtype=self.np_dtype)
+        q = np.ascontiguousarray(q, dtype=self.q_dtype)
         rows = int(qi[-1])
         assert q.shape == (rows, self.Hq, self.D)
         out = np.zeros((rows, self.Hq, self.D), np.float64)
@@ -204,7 +208,7 @@ class Oracle:
         return (out, lse) if check else (rc, out, lse)
 
     def attend_range(self, seq: int, h: int, q_row: np.ndarray, t0: int, t1: int, probs: bool = False):
-        q_row = np.ascontiguousarray(q_row, dtype=self.np_dtype)
+        q_row = np.ascontiguousarray(q_row, dtype=self.q_dtype)
         out = np.zeros(self.D, np.float64)
         lse = np.zeros(1, np.float64)
         p = np.zeros(max(0, t1 - t0), np.float64) if probs else None
@@ -213,7 +217,7 @@ class Oracle:
         return (out, float(lse[0]), p) if probs else (out, float(lse[0]))
 
     def cascade_row(self, seq: int, h: int, q_row: np.ndarray, split: int):
-        q_row = np.ascontiguousarray(q_row, dtype=self.np_dtype)
+        q_row = np.ascontiguousarray(q_row, dtype=self.q_dtype)
         out = np.zeros(self.D, np.float64)
         lse = np.zeros(1, np.float64)
         self._chk(lib().oracle_cascade_row(self._h, int(seq), int(h), _p(q_row), int(split), _p(out),
@@ -232,10 +236,9 @@ def merge2(oa: np.ndarray, lsea: float, ob: np.ndarray, lseb: float):
 
 def attend_dense(dtype: str, scale: float, q_row: np.ndarray, K: np.ndarray, V: np.ndarray):
     """Plain definition on an unpaged [n][D] K/V of one kv head (storage dtype)."""
-    npdt = np.float32 if dtype == "f32" else np.uint16
-    q_row = np.ascontiguousarray(q_row, dtype=npdt)
-    K = np.ascontiguousarray(K, dtype=npdt)
-    V = np.ascontiguousarray(V, dtype=npdt)
+    q_row = np.ascontiguousarray(q_row, dtype=Q_NP[dtype])
+    K = np.ascontiguousarray(K, dtype=KV_NP[dtype])
+    V = np.ascontiguousarray(V, dtype=KV_NP[dtype])
     n, D = K.shape
     out = np.zeros(D, np.float64)
     lse = np.zeros(1, np.float64)
@@ -244,6 +247,14 @@ def attend_dense(dtype: str, scale: float, q_row: np.ndarray, K: np.ndarray, V: 
     if rc != OK:
         raise OracleError(rc)
     return out, float(lse[0])
+
+
+def widen(dtype: str, a: np.ndarray) -> np.ndarray:
+    """The oracle's exact widening of stored K/V elements (bit patterns) to float64."""
+    a = np.ascontiguousarray(a, dtype=KV_NP[dtype])
+    out = np.zeros(a.shape, np.float64)
+    lib().oracle_widen(DTYPES[dtype], _p(a), a.size, _p(out))
+    return out
 
 
 def accept_len(q_indptr, draft_tokens, target_tokens) -> np.ndarray:

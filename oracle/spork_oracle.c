@@ -44,6 +44,13 @@
  * Storage: K/V/Q are kept in their storage dtype (fp32, or bf16 as uint16 bit
  * patterns rounded once by the input generator) and widened exactly to fp64
  * on every read.
+ *
+ * FP8-KV variant (ORACLE_E4M3KV, reading B-4):
+ * K and V are stored as e4m3 bytes (1 sign, 4 exponent bits with bias 7, 3
+ * mantissa bits; no infinities; exponent 15 with mantissa 7 is NaN; exponent 0
+ * is subnormal: m/8 * 2^-6), Q stays bf16.  Only the widening differs: the
+ * definition above is applied to the exactly widened values.  Pinned against
+ * torch.float8_e4m3fn -> float64 on all 256 codes (tests/test_oracle_fp8.py).
  */
 #include <math.h>
 #include <stdint.h>
@@ -60,6 +67,7 @@
 
 #define ORACLE_F32 0
 #define ORACLE_BF16 1
+#define ORACLE_E4M3KV 2   /* K, V: e4m3 bytes; Q: bf16 */
 
 typedef struct oracle_ctx {
     int dtype, Hq, Hkv, D, ps;
@@ -75,21 +83,41 @@ typedef struct oracle_ctx {
 } oracle_ctx;
 
 /* ---- exact widening ------------------------------------------------------ */
-static double load_elt(const oracle_ctx *c, const uint8_t *base, size_t idx) {
-    if (c->dtype == ORACLE_F32) {
-        float f;
-        memcpy(&f, base + idx * 4, 4);
-        return (double)f;
-    } else {
-        uint16_t h;
-        uint32_t u;
-        float f;
-        memcpy(&h, base + idx * 2, 2);
-        u = ((uint32_t)h) << 16;
-        memcpy(&f, &u, 4);
-        return (double)f;
-    }
+static double widen_f32(const uint8_t *base, size_t idx) {
+    float f;
+    memcpy(&f, base + idx * 4, 4);
+    return (double)f;
 }
+static double widen_bf16(const uint8_t *base, size_t idx) {
+    uint16_t h;
+    uint32_t u;
+    float f;
+    memcpy(&h, base + idx * 2, 2);
+    u = ((uint32_t)h) << 16;
+    memcpy(&f, &u, 4);
+    return (double)f;
+}
+/* e4m3 ("fn": finite + NaN): value = (-1)^s * 2^(e-7) * (1 + m/8), e = 1..15;
+ * e = 0: (-1)^s * 2^-6 * m/8; s.1111.111 is NaN */
+static double widen_e4m3(const uint8_t *base, size_t idx) {
+    uint8_t b = base[idx];
+    int sgn = b >> 7, e = (b >> 3) & 15, m = b & 7;
+    double v;
+    if (e == 15 && m == 7) return NAN;
+    v = e == 0 ? ldexp((double)m / 8.0, -6) : ldexp(1.0 + (double)m / 8.0, e - 7);
+    return sgn ? -v : v;
+}
+/* one stored K / V element */
+static double load_elt(const oracle_ctx *c, const uint8_t *base, size_t idx) {
+    if (c->dtype == ORACLE_F32) return widen_f32(base, idx);
+    if (c->dtype == ORACLE_BF16) return widen_bf16(base, idx);
+    return widen_e4m3(base, idx);
+}
+/* one stored Q element (the KV dtype, except for e4m3 KV, whose queries are bf16) */
+static double load_q(const oracle_ctx *c, const uint8_t *base, size_t idx) {
+    return c->dtype == ORACLE_F32 ? widen_f32(base, idx) : widen_bf16(base, idx);
+}
+static size_t q_elt(const oracle_ctx *c) { return c->dtype == ORACLE_F32 ? 4 : 2; }
 
 static size_t page_elems(const oracle_ctx *c) { return (size_t)c->Hkv * c->ps * c->D; }
 
@@ -102,14 +130,14 @@ oracle_ctx *oracle_create(int dtype, int Hq, int Hkv, int D, int ps, int num_pag
                           int max_pages_per_seq, double scale, int store_kv) {
     oracle_ctx *c;
     if (Hq <= 0 || Hkv <= 0 || D <= 0 || ps <= 0 || Hq % Hkv || num_pages <= 0 || max_seqs <= 0 ||
-        max_pages_per_seq <= 0 || (dtype != ORACLE_F32 && dtype != ORACLE_BF16))
+        max_pages_per_seq <= 0 || (dtype != ORACLE_F32 && dtype != ORACLE_BF16 && dtype != ORACLE_E4M3KV))
         return NULL;
     c = (oracle_ctx *)calloc(1, sizeof(*c));
     if (!c) return NULL;
     c->dtype = dtype; c->Hq = Hq; c->Hkv = Hkv; c->D = D; c->ps = ps;
     c->num_pages = num_pages; c->max_seqs = max_seqs; c->max_pages_per_seq = max_pages_per_seq;
     c->scale = scale; c->store_kv = store_kv;
-    c->elt = dtype == ORACLE_F32 ? 4 : 2;
+    c->elt = dtype == ORACLE_F32 ? 4 : (dtype == ORACLE_BF16 ? 2 : 1);
     c->refcount = (int32_t *)calloc((size_t)num_pages, sizeof(int32_t));
     c->table = (int32_t *)malloc((size_t)max_seqs * max_pages_per_seq * sizeof(int32_t));
     c->len = (int32_t *)calloc((size_t)max_seqs, sizeof(int32_t));
@@ -336,7 +364,7 @@ static int attend_range(const oracle_ctx *c, int seq, int h, const uint8_t *q, i
     for (t = 0; t < n; ++t) {                        /* s_t = scale * <q, k_t> */
         size_t ki = kv_index(c, tab[(t0 + t) / c->ps], kvh, (t0 + t) % c->ps);
         double acc = 0.0;
-        for (d = 0; d < D; ++d) acc += load_elt(c, q, (size_t)d) * load_elt(c, c->kpool, ki + d);
+        for (d = 0; d < D; ++d) acc += load_q(c, q, (size_t)d) * load_elt(c, c->kpool, ki + d);
         s[t] = c->scale * acc;
         if (s[t] > m) m = s[t];
     }
@@ -363,7 +391,7 @@ int oracle_decode(const oracle_ctx *c, int n, const int32_t *seq_ids, const void
 #pragma omp parallel for schedule(dynamic, 1)
     for (i = 0; i < n * c->Hq; ++i) {
         int si = i / c->Hq, h = i % c->Hq, s = seq_ids[si];
-        const uint8_t *qr = (const uint8_t *)q + ((size_t)si * c->Hq + h) * c->D * c->elt;
+        const uint8_t *qr = (const uint8_t *)q + ((size_t)si * c->Hq + h) * c->D * q_elt(c);
         int r = attend_range(c, s, h, qr, 0, c->len[s], out + ((size_t)si * c->Hq + h) * c->D,
                              lse + (size_t)si * c->Hq + h, NULL);
         if (r != ORACLE_OK) rc = r;
@@ -387,7 +415,7 @@ int oracle_verify(const oracle_ctx *c, int n, const int32_t *seq_ids, const int3
 #pragma omp parallel for schedule(dynamic, 1)
     for (i = 0; i < rows; ++i) {
         int row = i / c->Hq, h = i % c->Hq, si = 0, s, k, j, r;
-        const uint8_t *qr = (const uint8_t *)q + (size_t)i * c->D * c->elt;
+        const uint8_t *qr = (const uint8_t *)q + (size_t)i * c->D * q_elt(c);
         while (q_indptr[si + 1] <= row) ++si;
         s = seq_ids[si]; k = q_indptr[si + 1] - q_indptr[si]; j = row - q_indptr[si];
         r = attend_range(c, s, h, qr, 0, c->len[s] - k + j + 1, out + (size_t)i * c->D, lse + i, NULL);
@@ -461,7 +489,7 @@ int oracle_attend_dense(int dtype, int D, double scale, const void *q_row, const
     for (t = 0; t < n; ++t) {
         double acc = 0.0;
         for (d = 0; d < D; ++d)
-            acc += load_elt(&tmp, (const uint8_t *)q_row, (size_t)d) *
+            acc += load_q(&tmp, (const uint8_t *)q_row, (size_t)d) *
                    load_elt(&tmp, (const uint8_t *)K, (size_t)t * D + d);
         s[t] = scale * acc;
         if (s[t] > m) m = s[t];
@@ -474,6 +502,15 @@ int oracle_attend_dense(int dtype, int D, double scale, const void *q_row, const
     *lse = m + log(Z);
     free(s);
     return ORACLE_OK;
+}
+
+/* exact widening of n stored K/V elements (for the pins of the storage formats) */
+void oracle_widen(int dtype, const void *src, long n, double *out) {
+    oracle_ctx tmp;
+    long i;
+    memset(&tmp, 0, sizeof(tmp));
+    tmp.dtype = dtype;
+    for (i = 0; i < n; ++i) out[i] = load_elt(&tmp, (const uint8_t *)src, (size_t)i);
 }
 
 int oracle_num_threads(void) {

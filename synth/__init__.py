@@ -63,12 +63,38 @@ def bf16_bits_to_f32(u: np.ndarray) -> np.ndarray:
     return (u.astype(np.uint32) << np.uint32(16)).view(np.float32)
 
 
+def f32_to_e4m3_bits(x: np.ndarray) -> np.ndarray:
+    """float32 -> e4m3 ("fn") bit pattern (uint8): round-to-nearest-even, saturating at +-448.
+    Format: 1 sign, 4 exponent bits (bias 7), 3 mantissa bits; exponent 0 is subnormal (m/8 * 2^-6)."""
+    x = np.ascontiguousarray(x, dtype=np.float32).astype(np.float64)
+    a = np.minimum(np.abs(x), 448.0)
+    _, e = np.frexp(a)                           # a = f * 2^e, f in [0.5, 1)
+    quantum = np.ldexp(1.0, np.maximum(e - 1, -6) - 3)   # spacing of the format at a (2^-9 below 2^-6)
+    q = np.minimum(np.rint(a / quantum) * quantum, 448.0)   # np.rint: ties to even
+    _, e2 = np.frexp(q)
+    eb = np.where(q >= 2.0 ** -6, e2 - 1 + 7, 0)
+    m = np.where(eb > 0, (q / np.ldexp(1.0, eb - 7) - 1.0) * 8.0, q / 2.0 ** -9)
+    bits = (eb.astype(np.int64) << 3) | m.astype(np.int64) | (np.signbit(x).astype(np.int64) << 7)
+    return bits.astype(np.uint8)
+
+
+def e4m3_bits_to_f32(u: np.ndarray) -> np.ndarray:
+    """e4m3 bit pattern (uint8) -> float32 (exact; 0x7f / 0xff are NaN)."""
+    u = np.ascontiguousarray(u, dtype=np.uint8).astype(np.int64)
+    e, m = (u >> 3) & 15, u & 7
+    v = np.where(e == 0, np.ldexp(m / 8.0, -6), np.ldexp(1.0 + m / 8.0, e - 7))
+    v = np.where((e == 15) & (m == 7), np.nan, v)
+    return np.where(u >> 7, -v, v).astype(np.float32)
+
+
 def to_storage(x: np.ndarray, dtype: str) -> np.ndarray:
-    """Round float32 values once to the storage dtype ('f32' or 'bf16')."""
+    """Round float32 values once to the storage dtype ('f32', 'bf16' or 'e4m3')."""
     if dtype == "f32":
         return np.ascontiguousarray(x, dtype=np.float32)
     if dtype == "bf16":
         return f32_to_bf16_bits(x)
+    if dtype == "e4m3":
+        return f32_to_e4m3_bits(x)
     raise ValueError(dtype)
 
 
@@ -78,11 +104,18 @@ def storage_to_f64(x: np.ndarray, dtype: str) -> np.ndarray:
         return np.asarray(x, dtype=np.float32).astype(np.float64)
     if dtype == "bf16":
         return bf16_bits_to_f32(x).astype(np.float64)
+    if dtype == "e4m3":
+        return e4m3_bits_to_f32(x).astype(np.float64)
     raise ValueError(dtype)
 
 
 def storage_np_dtype(dtype: str):
-    return np.float32 if dtype == "f32" else np.uint16
+    return {"f32": np.float32, "bf16": np.uint16, "e4m3": np.uint8}[dtype]
+
+
+def q_dtype_of(dtype: str) -> str:
+    """Storage dtype of the queries: the KV dtype, except that an e4m3 KV cache is queried in bf16."""
+    return "bf16" if dtype == "e4m3" else dtype
 
 
 # ----------------------------------------------------------------------------
@@ -92,7 +125,7 @@ def storage_np_dtype(dtype: str):
 class SporkConfig:
     name: str
     cfg_no: int
-    dtype: str            # 'f32' | 'bf16'  (KV and Q storage dtype)
+    dtype: str            # 'f32' | 'bf16' (KV and Q storage dtype) | 'e4m3' (KV; Q is bf16)
     Hq: int
     Hkv: int
     D: int
@@ -120,7 +153,11 @@ class SporkConfig:
 
     @property
     def elt_bytes(self) -> int:
-        return 4 if self.dtype == "f32" else 2
+        return {"f32": 4, "bf16": 2, "e4m3": 1}[self.dtype]
+
+    @property
+    def q_dtype(self) -> str:
+        return q_dtype_of(self.dtype)
 
     @property
     def token_bytes(self) -> int:
@@ -235,7 +272,7 @@ class Workload:
         """query rows of one sequence, storage dtype, [q_rows][Hq][D]."""
         c = self.cfg
         n = int(self.q_rows()[seq])
-        return to_storage(self._normal(T_Q, seq, n, c.Hq), c.dtype)
+        return to_storage(self._normal(T_Q, seq, n, c.Hq), c.q_dtype)
 
     def q_all(self) -> np.ndarray:
         return np.concatenate([self.q(i) for i in range(self.cfg.n_seqs)], axis=0)
