@@ -60,11 +60,15 @@ extern "C" {
 
 #define SPORK_F32 0
 #define SPORK_BF16 1
+#define SPORK_E4M3 2   /* FP8-KV variant (reading B-4): K and V are e4m3
+                          bytes ("fn": bias 7, subnormals, no infinities, s.1111.111 = NaN); Q is BF16 */
 
 typedef struct spork_ctx spork_ctx;
 
 typedef struct spork_config {
-    int32_t dtype;             /* SPORK_F32 | SPORK_BF16: storage type of K, V and Q    */
+    int32_t dtype;             /* SPORK_F32 | SPORK_BF16: storage type of K, V and Q;
+                                  SPORK_E4M3: K and V are e4m3 bytes, Q is bf16 (queries
+                                  beyond fp16's range, |q| > 65504, saturate there)        */
     int32_t num_q_heads;       /* Hq                                                    */
     int32_t num_kv_heads;      /* Hkv, divides Hq; q head h reads kv head h/(Hq/Hkv)    */
     int32_t head_dim;          /* D: multiple of 32, <= 256                             */
@@ -75,7 +79,7 @@ typedef struct spork_config {
     float scale;               /* softmax scale (1/sqrt(D)); scores = scale * <q,k>     */
 } spork_config;
 
-/* Bytes of one page in ONE pool (K or V): Hkv * 16 * D * sizeof(dtype). */
+/* Bytes of one page in ONE pool (K or V): Hkv * 16 * D * sizeof(K/V element). */
 size_t spork_page_bytes(const spork_config *cfg);
 
 /*
@@ -84,8 +88,8 @@ size_t spork_page_bytes(const spork_config *cfg);
  * num_pages * spork_page_bytes() bytes, 256-byte aligned, contents arbitrary.
  * Logical layout of a pool is [num_pages][Hkv][16][D]; the arrangement of the
  * 16 x D elements inside one (page, kv head) block is library-defined (for
- * bf16 with D % 64 == 0 it is the 128-byte-swizzled shared-memory image the
- * attention kernels consume, so a block is staged with one bulk copy).  Write
+ * bf16 with D % 64 == 0, and for e4m3 with D % 128 == 0, it is a 128-byte-swizzled
+ * shared-memory image, so a block is staged with one bulk copy).  Write
  * pools only through spork_append / spork_fork; read them through
  * spork_read_kv.  The library owns block tables, refcounts and workspace.
  * Errors: SPORK_ERR_INVALID (shapes), SPORK_ERR_CUDA.

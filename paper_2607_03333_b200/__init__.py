@@ -19,7 +19,7 @@ import numpy as np
 
 from . import build as _build
 
-F32, BF16 = 0, 1
+F32, BF16, E4M3 = 0, 1, 2
 PAGE_SIZE = 16
 
 OK = 0
@@ -147,9 +147,11 @@ class Spork:
         self.num_pages, self.max_seqs, self.max_pages_per_seq = num_pages, max_seqs, max_pages_per_seq
         self.scale = float(scale)
         self.ps = PAGE_SIZE
-        self.np_dtype = np.float32 if dtype == "f32" else np.uint16
+        # host arrays are bit patterns: K / V in np_dtype, queries in q_np_dtype ("e4m3": fp8 cache, bf16 queries)
+        self.np_dtype = {"f32": np.float32, "bf16": np.uint16, "e4m3": np.uint8}[dtype]
+        self.q_np_dtype = np.float32 if dtype == "f32" else np.uint16
         self.torch_dtype = torch.float32 if dtype == "f32" else torch.bfloat16
-        self.cfg = SporkConfig({"f32": F32, "bf16": BF16}[dtype], Hq, Hkv, D, PAGE_SIZE, num_pages,
+        self.cfg = SporkConfig({"f32": F32, "bf16": BF16, "e4m3": E4M3}[dtype], Hq, Hkv, D, PAGE_SIZE, num_pages,
                                max_seqs, max_pages_per_seq, self.scale)
         self.page_bytes = int(self.lib.spork_page_bytes(C.byref(self.cfg)))
         # caller-owned pools: raw bytes (torch.empty: contents arbitrary on purpose)
@@ -223,7 +225,7 @@ class Spork:
         kd = k if hasattr(k, "data_ptr") else self._dev(np.asarray(k, dtype=self.np_dtype))
         vd = v if hasattr(v, "data_ptr") else self._dev(np.asarray(v, dtype=self.np_dtype))
         total = int(nt[nt > 0].sum()) if len(nt) else 0
-        assert kd.numel() * kd.element_size() == total * self.Hkv * self.D * (4 if self.dtype == "f32" else 2)
+        assert kd.numel() * kd.element_size() == total * self.Hkv * self.D * np.dtype(self.np_dtype).itemsize
         self._enter()
         rc = self.lib.spork_append(self._h, len(s), _p(s), _p(nt), kd.data_ptr(), vd.data_ptr(), self._st)
         self._hold(kd, vd)
@@ -282,7 +284,7 @@ class Spork:
         Returns device fp32 tensors (out [n_seq][Hq][D], lse [n_seq][Hq])."""
         torch = self.torch
         gi, s = _i32(group_indptr), _i32(seq_ids)
-        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.np_dtype))
+        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.q_np_dtype))
         n = len(s)
         if out is None:
             out = torch.empty((n, self.Hq, self.D), dtype=torch.float32, device=self.device)
@@ -299,7 +301,7 @@ class Spork:
     def verify_attn(self, group_indptr, seq_ids, q_indptr, q, out=None, lse=None, check: bool = True):
         torch = self.torch
         gi, s, qi = _i32(group_indptr), _i32(seq_ids), _i32(q_indptr)
-        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.np_dtype))
+        qd = q if hasattr(q, "data_ptr") else self._dev(np.asarray(q, dtype=self.q_np_dtype))
         rows = int(qi[-1]) if len(qi) else 0
         if out is None:
             out = torch.empty((rows, self.Hq, self.D), dtype=torch.float32, device=self.device)

@@ -66,7 +66,7 @@ int devbuf_reserve(DevBuf *b, size_t bytes, cudaStream_t st) {
 // ---------------------------------------------------------------------------
 extern "C" size_t spork_page_bytes(const spork_config *cfg) {
     if (!cfg) return 0;
-    size_t elt = cfg->dtype == SPORK_F32 ? 4 : 2;
+    size_t elt = cfg->dtype == SPORK_F32 ? 4 : (cfg->dtype == SPORK_E4M3 ? 1 : 2);
     return (size_t)cfg->num_kv_heads * PS * cfg->head_dim * elt;
 }
 
@@ -100,7 +100,7 @@ __global__ void init_state_kernel(int32_t *refcount, int num_pages, int32_t *tab
 
 extern "C" int spork_create(const spork_config *cfg, void *k_pool, void *v_pool, spork_ctx **out) {
     if (!cfg || !out || !k_pool || !v_pool) return SPORK_ERR_INVALID;
-    if (cfg->dtype != SPORK_F32 && cfg->dtype != SPORK_BF16) return SPORK_ERR_INVALID;
+    if (cfg->dtype != SPORK_F32 && cfg->dtype != SPORK_BF16 && cfg->dtype != SPORK_E4M3) return SPORK_ERR_INVALID;
     if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_q_heads % cfg->num_kv_heads)
         return SPORK_ERR_INVALID;
     if (cfg->head_dim <= 0 || cfg->head_dim % 32 || cfg->head_dim > 256) return SPORK_ERR_INVALID;
@@ -113,8 +113,9 @@ extern "C" int spork_create(const spork_config *cfg, void *k_pool, void *v_pool,
     if (!c) return SPORK_ERR_INVALID;
     c->cfg = *cfg;
     c->G = cfg->num_q_heads / cfg->num_kv_heads;
-    c->elt = cfg->dtype == SPORK_F32 ? 4 : 2;
-    c->swizzled = (cfg->dtype == SPORK_BF16 && cfg->head_dim % 64 == 0) ? 1 : 0;
+    c->elt = cfg->dtype == SPORK_F32 ? 4 : (cfg->dtype == SPORK_E4M3 ? 1 : 2);
+    c->q_elt = cfg->dtype == SPORK_F32 ? 4 : 2;
+    c->swizzled = (cfg->dtype != SPORK_F32 && cfg->head_dim * c->elt % 128 == 0) ? 1 : 0;
     c->head_block = (size_t)PS * cfg->head_dim * c->elt;
     c->page_bytes = c->head_block * cfg->num_kv_heads;
     c->table_stride = (cfg->max_pages_per_seq + 3) & ~3;
@@ -268,7 +269,7 @@ __global__ void read_kv_kernel(const T *__restrict__ kpool, const T *__restrict_
         int h = (int)((i / D) % Hkv);
         int t = t0 + (int)(i / ((size_t)D * Hkv));
         int page = table_row[t / PS];
-        size_t off = ((size_t)page * Hkv + h) * (size_t)(PS * D) + head_block_off(swizzled, D, t % PS, d);
+        size_t off = ((size_t)page * Hkv + h) * (size_t)(PS * D) + head_block_off(swizzled, D, (int)sizeof(T), t % PS, d);
         k_out[i] = kpool[off];
         v_out[i] = vpool[off];
     }
@@ -293,6 +294,10 @@ extern "C" int spork_read_kv(spork_ctx *c, int32_t seq, int32_t t0, int32_t n, v
         read_kv_kernel<float><<<256, 256>>>((const float *)c->k_pool, (const float *)c->v_pool, row, t0,
                                             n, c->cfg.num_kv_heads, c->cfg.head_dim, c->swizzled,
                                             (float *)dk, (float *)dv);
+    else if (c->elt == 1)
+        read_kv_kernel<uint8_t><<<256, 256>>>((const uint8_t *)c->k_pool, (const uint8_t *)c->v_pool, row, t0,
+                                              n, c->cfg.num_kv_heads, c->cfg.head_dim, c->swizzled,
+                                              (uint8_t *)dk, (uint8_t *)dv);
     else
         read_kv_kernel<uint16_t><<<256, 256>>>((const uint16_t *)c->k_pool,
                                                (const uint16_t *)c->v_pool, row, t0, n,

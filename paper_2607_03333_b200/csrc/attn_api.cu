@@ -135,7 +135,7 @@ static int attn_host(spork_ctx *c, int n_groups, const int32_t *group_indptr, co
     const int n_seq = group_indptr[n_groups];
     const size_t rows = q_indptr ? (size_t)q_indptr[n_seq] : (size_t)n_seq;
     const size_t Hq = c->cfg.num_q_heads, D = c->cfg.head_dim;
-    const size_t qb = rows * Hq * D * c->elt, ob = rows * Hq * D * 4, lb = rows * Hq * 4;
+    const size_t qb = rows * Hq * D * c->q_elt, ob = rows * Hq * D * 4, lb = rows * Hq * 4;
     if (rows == 0) return SPORK_OK;
     if (!q_host || !out_host || !lse_host) return SPORK_ERR_INVALID;
     int rc = devbuf_reserve(&c->io_q, qb, st);

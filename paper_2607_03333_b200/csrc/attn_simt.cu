@@ -1,4 +1,4 @@
-// libspork: generic CUDA-core attention kernel (fp32 KV, or bf16 with D != 128)
+// libspork: generic CUDA-core attention kernel (fp32 KV, or bf16 / e4m3 KV with D != 128)
 // and the LSE merge kernel shared by both attention paths.
 //
 // simt kernel: one CTA per work item, one warp per query row at a time.  A
@@ -6,6 +6,7 @@
 // D/32 output dims for the value pass.  fp32 accumulation, accurate expf/logf:
 // this is the path that has to meet 1e-5 on fp32 KV (config 1), not a
 // bandwidth target.
+#include <cuda_fp16.h>
 #include <math.h>
 
 #include "spork_internal.h"
@@ -46,6 +47,22 @@ template <> struct Elt<uint16_t> {
     }
 };
 
+// e4m3 ("fn") byte -> fp32, exact: the byte's magnitude bits shifted into an fp16 pattern read 2^-8 too
+// small (subnormals included); s.1111.111 is NaN
+__device__ __forceinline__ float e4m3_to_f32(uint32_t b) {
+    const float v = __half2float(__ushort_as_half((unsigned short)(((b & 0x80u) << 8) | ((b & 0x7fu) << 7)))) * 256.f;
+    return (b & 0x7fu) == 0x7fu ? __int_as_float(0x7fffffff) : v;
+}
+template <> struct Elt<uint8_t> {
+    static constexpr int PER_CHUNK = 16;
+    static __device__ __forceinline__ void unpack(const uint4 &v, float *f) {
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int i = 0; i < 16; ++i) f[i] = e4m3_to_f32((w[i >> 2] >> (8 * (i & 3))) & 0xffu);
+    }
+    static __device__ __forceinline__ float load(const uint8_t *p) { return e4m3_to_f32(*p); }
+};
+
 __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
     for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
@@ -57,10 +74,11 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-template <typename T, int DMAX>
+// T: stored K / V element, TQ: stored Q element (the same type, except e4m3 KV with bf16 queries)
+template <typename T, typename TQ, int DMAX>
 __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
     const WorkItem *__restrict__ items, const int32_t *__restrict__ seq_len,
-    const int32_t *__restrict__ rowmap, const T *__restrict__ q, const uint8_t *__restrict__ k_pool,
+    const int32_t *__restrict__ rowmap, const TQ *__restrict__ q, const uint8_t *__restrict__ k_pool,
     const uint8_t *__restrict__ v_pool, const int32_t *__restrict__ table, int table_stride, int Hq,
     int Hkv, int G, int D, int swizzled, float scale, float *__restrict__ ws_o,
     float *__restrict__ ws_lse) {
@@ -79,7 +97,7 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
         const int lim = it.lim0 + lr / G;
         __syncwarp();
         for (int d = lane; d < D; d += 32)
-            qs[warp][d] = Elt<T>::load(reinterpret_cast<const uint8_t *>(q + ((size_t)qrow * Hq + h) * D + d));
+            qs[warp][d] = Elt<TQ>::load(reinterpret_cast<const uint8_t *>(q + ((size_t)qrow * Hq + h) * D + d));
         __syncwarp();
         float m = -INFINITY, l = 0.f, acc[NACC];
 #pragma unroll
@@ -209,19 +227,23 @@ int launch_attn_simt(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
     const uint8_t *kp = (const uint8_t *)io.k_pool, *vp = (const uint8_t *)io.v_pool;
     const spork_config &f = c->cfg;
     dim3 grid(P.n_items), block(SIMT_WARPS * 32);
-#define SPORK_SIMT(T, DMAX)                                                                        \
-    attn_simt_kernel<T, DMAX><<<grid, block, 0, st>>>(items, c->d_len, P.d_rowmap, (const T *)io.q, kp, vp, \
-                                                      c->d_table, c->table_stride, f.num_q_heads,  \
-                                                      f.num_kv_heads, c->G, f.head_dim,            \
-                                                      c->swizzled, f.scale, wo, wl)
+#define SPORK_SIMT(T, TQ, DMAX)                                                                    \
+    attn_simt_kernel<T, TQ, DMAX><<<grid, block, 0, st>>>(items, c->d_len, P.d_rowmap, (const TQ *)io.q, kp, vp, \
+                                                          c->d_table, c->table_stride, f.num_q_heads, \
+                                                          f.num_kv_heads, c->G, f.head_dim,        \
+                                                          c->swizzled, f.scale, wo, wl)
     if (f.dtype == SPORK_F32) {
-        if (f.head_dim <= 64) SPORK_SIMT(float, 64);
-        else if (f.head_dim <= 128) SPORK_SIMT(float, 128);
-        else SPORK_SIMT(float, 256);
+        if (f.head_dim <= 64) SPORK_SIMT(float, float, 64);
+        else if (f.head_dim <= 128) SPORK_SIMT(float, float, 128);
+        else SPORK_SIMT(float, float, 256);
+    } else if (f.dtype == SPORK_E4M3) {
+        if (f.head_dim <= 64) SPORK_SIMT(uint8_t, uint16_t, 64);
+        else if (f.head_dim <= 128) SPORK_SIMT(uint8_t, uint16_t, 128);
+        else SPORK_SIMT(uint8_t, uint16_t, 256);
     } else {
-        if (f.head_dim <= 64) SPORK_SIMT(uint16_t, 64);
-        else if (f.head_dim <= 128) SPORK_SIMT(uint16_t, 128);
-        else SPORK_SIMT(uint16_t, 256);
+        if (f.head_dim <= 64) SPORK_SIMT(uint16_t, uint16_t, 64);
+        else if (f.head_dim <= 128) SPORK_SIMT(uint16_t, uint16_t, 128);
+        else SPORK_SIMT(uint16_t, uint16_t, 256);
     }
 #undef SPORK_SIMT
     c->last_launches++;

@@ -58,25 +58,36 @@ __host__ __device__ constexpr bool emulated_pair(int j) { return (j * EMU_NUM) %
 //   SP = 2 (NP = 1 only): every row's 64 scores of a tile are split over TWO threads (8 softmax warps,
 //           4 per SM sub-partition instead of 2) for items whose time is the softmax's, not HBM's:
 //           4-slot ring, the row max and the row sums are exchanged through shared memory
-template <int NP, int SP>
+//   F8 (NP = SP = 1): the FP8-KV variant (e4m3 K/V bytes, bf16 Q).  The bulk copies land 8 KiB e4m3 tiles
+//           in a 6-slot ring; two converter warps widen them (exactly) to fp16 into ONE K operand slot and
+//           ONE V operand slot in the same swizzled image the bf16 path stages directly, Q is converted
+//           bf16 -> fp16 when it is staged, P is packed as fp16: the MMAs run in kind::f16 with fp16
+//           operands, everything downstream of the operands is the bf16 kernel.
+template <int NP, int SP, bool F8 = false>
 struct Cfg {
     static_assert(SP == 1 || NP == 1, "split rows only with one pipe");
-    static constexpr int NSLOT = NP == 2 ? 10 : (SP == 2 ? 4 : 5);
+    static_assert(!F8 || (NP == 1 && SP == 1), "FP8-KV: the default kernel shape only");
+    static constexpr int NSLOT = F8 ? 6 : (NP == 2 ? 10 : (SP == 2 ? 4 : 5));
+    static constexpr int RING_SLOT = F8 ? SLOT_BYTES / 2 : SLOT_BYTES;   // bytes of one landed K or V tile
     static constexpr int N_SOFTMAX = NP * 128 * SP;
-    static constexpr int N_THREADS = 64 + N_SOFTMAX;
+    static constexpr int N_CONV = F8 ? 64 : 0;                            // converter threads (2 warps)
+    static constexpr int N_THREADS = 64 + N_SOFTMAX + N_CONV;
     static constexpr int CTAS_PER_SM = NP == 1 ? 2 : 1;
     static constexpr int TMEM_COLS = NP * PIPE_COLS;
-    static constexpr int RING_OFF = NP * Q_BYTES;
-    static constexpr int BAR_OFF = RING_OFF + NSLOT * SLOT_BYTES;
+    static constexpr int OPER_OFF = NP * Q_BYTES;                         // F8: fp16 K slot, then fp16 V slot
+    static constexpr int RING_OFF = OPER_OFF + (F8 ? 2 * SLOT_BYTES : 0);
+    static constexpr int BAR_OFF = RING_OFF + NSLOT * RING_SLOT;
     // barrier slots (8 bytes each) from BAR_OFF
     static constexpr int B_FULL = 0;                  // [NSLOT] bulk copies landed
-    static constexpr int B_EMPTY = NSLOT;             // [NSLOT] MMAs reading the slot completed
+    static constexpr int B_EMPTY = NSLOT;             // [NSLOT] MMAs (F8: converters) reading the slot completed
     static constexpr int B_PIPE = 2 * NSLOT;          // per pipe: 7 barriers, see P_*
     static constexpr int B_QFULL = B_PIPE + 7 * NP;   // Q staged
-    static constexpr int B_COUNT = B_QFULL + 1;
+    static constexpr int B_OPER = B_QFULL + 1;        // F8: K slot full / empty, V slot full / empty
+    static constexpr int B_COUNT = B_OPER + (F8 ? 4 : 0);
     static constexpr int XCH_OFF = BAR_OFF + 8 * B_COUNT + 16;     // float [2][2][128] (SP = 2)
     static constexpr int SMEM_BYTES = XCH_OFF + (SP == 2 ? 2048 : 0);
 };
+enum : int { O_KFULL = 0, O_KEMPTY = 1, O_VFULL = 2, O_VEMPTY = 3 };
 enum : int {
     P_SFULL = 0,    // [2] S(b) complete
     P_PFULL = 2,    // [2] P(b) written (4 softmax warps)
@@ -99,10 +110,10 @@ struct UParams {
                                   // (the merge of the previous layer): wait for it before the first partial
 };
 
-template <int NP, int SP>
-__global__ void __launch_bounds__(Cfg<NP, SP>::N_THREADS, Cfg<NP, SP>::CTAS_PER_SM)
+template <int NP, int SP, bool F8>
+__global__ void __launch_bounds__(Cfg<NP, SP, F8>::N_THREADS, Cfg<NP, SP, F8>::CTAS_PER_SM)
 attn_umma_kernel(const UParams P) {
-    using C = Cfg<NP, SP>;
+    using C = Cfg<NP, SP, F8>;
     constexpr int NSLOT = C::NSLOT;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = smem_u32(smem);
@@ -117,7 +128,7 @@ attn_umma_kernel(const UParams P) {
         if (sbase & 1023u) __trap();   // the 128-byte swizzle is a function of the smem address
         for (int s = 0; s < NSLOT; ++s) {
             mbar_init(bar(C::B_FULL + s), 1);
-            mbar_init(bar(C::B_EMPTY + s), 1);
+            mbar_init(bar(C::B_EMPTY + s), F8 ? 2 : 1);
         }
         for (int w = 0; w < NP; ++w) {
             for (int b = 0; b < 2; ++b) {
@@ -128,6 +139,12 @@ attn_umma_kernel(const UParams P) {
             mbar_init(pbar(w, P_OFREE), 4 * SP);
         }
         mbar_init(bar(C::B_QFULL), 1);
+        if constexpr (F8) {
+            mbar_init(bar(C::B_OPER + O_KFULL), 2);     // one arrival per converter warp
+            mbar_init(bar(C::B_OPER + O_VFULL), 2);
+            mbar_init(bar(C::B_OPER + O_KEMPTY), 1);    // tcgen05.commit
+            mbar_init(bar(C::B_OPER + O_VEMPTY), 1);
+        }
         mbar_fence_init();
     }
     if (warp == 1) {
@@ -151,8 +168,9 @@ attn_umma_kernel(const UParams P) {
             const int n_pages = (it.tok1 + PS - 1) / PS - page0;
             const int n_tiles = (n_pages + TILE_PAGES - 1) / TILE_PAGES;
             const int32_t *row = P.table + (size_t)it.table_seq * P.table_stride + page0;
-            const size_t head_off = (size_t)it.kvh * HEAD_BLOCK;
-            const size_t page_stride = (size_t)P.Hkv * HEAD_BLOCK;
+            constexpr int HB = F8 ? HEAD_BLOCK / 2 : HEAD_BLOCK;     // bytes of a (page, kv head) block in the pool
+            const size_t head_off = (size_t)it.kvh * HB;
+            const size_t page_stride = (size_t)P.Hkv * HB;
             int e0 = 0, e1 = 0, e2 = 0, e3 = 0;
             for (int tile = 0; tile < n_tiles; ++tile) {
                 if ((tile & 31) == 0) {      // each lane fetches the 4 table entries of one tile
@@ -172,14 +190,14 @@ attn_umma_kernel(const UParams P) {
                     for (int kv = 0; kv < 2; ++kv) {
                         const uint32_t slot = (ld + kv) % NSLOT, ph = ((ld + kv) / NSLOT) & 1;
                         mbar_wait(bar(C::B_EMPTY + slot), ph ^ 1);
-                        mbar_expect_tx(bar(C::B_FULL + slot), (uint32_t)np * HEAD_BLOCK);
-                        const uint32_t dst = ring + slot * SLOT_BYTES;
+                        mbar_expect_tx(bar(C::B_FULL + slot), (uint32_t)np * HB);
+                        const uint32_t dst = ring + slot * C::RING_SLOT;
                         const uint8_t *pool = kv ? P.v_pool : P.k_pool;
 #pragma unroll
                         for (int p = 0; p < TILE_PAGES; ++p)
                             if (p < np)
-                                bulk_g2s(dst + p * HEAD_BLOCK, pool + (size_t)pg[p] * page_stride + head_off,
-                                         HEAD_BLOCK, bar(C::B_FULL + slot));
+                                bulk_g2s(dst + p * HB, pool + (size_t)pg[p] * page_stride + head_off,
+                                         HB, bar(C::B_FULL + slot));
                     }
                 }
                 ld += 2;
@@ -190,9 +208,11 @@ attn_umma_kernel(const UParams P) {
         // The whole warp runs this loop in lockstep (waits, counters, descriptors stay warp-uniform);
         // one elected lane issues the tcgen05 instructions of a step.
         const uint64_t q_desc = smem_desc_sw128(sbase, 16, 1024);     // K-major, 8-row groups 1 KiB apart
-        const uint64_t k_desc = smem_desc_sw128(ring, 16, 2048);      // K-major, 8-token groups 2 KiB apart
-        const uint64_t v_desc = smem_desc_sw128(ring, 1024, 2048);    // MN-major: dim halves 1 KiB, 8-token groups 2 KiB
-        constexpr uint32_t ID_PV = idesc_bf16(128, D, 0, 1);
+        // operand tiles: the ring itself, or (F8) the two fp16 slots the converter warps fill
+        const uint32_t k_base = F8 ? sbase + C::OPER_OFF : ring, v_base = F8 ? sbase + C::OPER_OFF + SLOT_BYTES : ring;
+        const uint64_t k_desc = smem_desc_sw128(k_base, 16, 2048);      // K-major, 8-token groups 2 KiB apart
+        const uint64_t v_desc = smem_desc_sw128(v_base, 1024, 2048);    // MN-major: dim halves 1 KiB, 8-token groups 2 KiB
+        constexpr uint32_t ID_PV = F8 ? idesc_f16(128, D, 0, 1) : idesc_bf16(128, D, 0, 1);
         uint32_t gt = 0;            // tiles of all items so far: K of tile gt is load 2 gt, V is 2 gt + 1
         uint32_t g0[NP];            // tiles pipe w has run (its S/P buffer and barrier phases)
         int jw[NP];                 // items pipe w has run
@@ -209,10 +229,12 @@ attn_umma_kernel(const UParams P) {
             };
             auto issue_s = [&](int i) {
                 const uint32_t ldk = 2 * (gt + i);
-                const uint32_t slot = ldk % NSLOT, ph = (ldk / NSLOT) & 1;
-                mbar_wait(bar(C::B_FULL + slot), ph);
+                const uint32_t slot = F8 ? 0 : ldk % NSLOT, ph = F8 ? (gt + i) & 1 : (ldk / NSLOT) & 1;
+                const uint32_t k_full = F8 ? bar(C::B_OPER + O_KFULL) : bar(C::B_FULL + slot);
+                const uint32_t k_empty = F8 ? bar(C::B_OPER + O_KEMPTY) : bar(C::B_EMPTY + slot);
+                mbar_wait(k_full, ph);
                 tc_fence_after();
-                const uint32_t id = idesc_bf16(128, PS * pages_of_tile(i), 0, 0);
+                const uint32_t id = F8 ? idesc_f16(128, PS * pages_of_tile(i), 0, 0) : idesc_bf16(128, PS * pages_of_tile(i), 0, 0);
                 const uint64_t kd = smem_desc_advance(k_desc, slot * SLOT_BYTES);
                 if (elect_one()) {
 #pragma unroll
@@ -227,7 +249,7 @@ attn_umma_kernel(const UParams P) {
                             mma_commit(pbar(w, P_SFULL + b));
                         }
                     }
-                    mma_commit(bar(C::B_EMPTY + slot));
+                    mma_commit(k_empty);
                 }
                 __syncwarp();
             };
@@ -237,7 +259,9 @@ attn_umma_kernel(const UParams P) {
             for (int i = 0; i < n_tiles; ++i) {
                 if (i + 1 < n_tiles) issue_s(i + 1);
                 const uint32_t ldv = 2 * (gt + i) + 1;
-                const uint32_t slot = ldv % NSLOT, ph = (ldv / NSLOT) & 1;
+                const uint32_t slot = F8 ? 0 : ldv % NSLOT, ph = F8 ? (gt + i) & 1 : (ldv / NSLOT) & 1;
+                const uint32_t v_full = F8 ? bar(C::B_OPER + O_VFULL) : bar(C::B_FULL + slot);
+                const uint32_t v_empty = F8 ? bar(C::B_OPER + O_VEMPTY) : bar(C::B_EMPTY + slot);
                 const uint64_t vd = smem_desc_advance(v_desc, slot * SLOT_BYTES);
                 const int nvp = pages_of_tile(i);
 #pragma unroll
@@ -245,7 +269,7 @@ attn_umma_kernel(const UParams P) {
                     if (w < npipe) {
                         const uint32_t g = g0[w] + i, b = g & 1;
                         mbar_wait(pbar(w, P_PFULL + b), (g >> 1) & 1);
-                        if (w == 0) mbar_wait(bar(C::B_FULL + slot), ph);
+                        if (w == 0) mbar_wait(v_full, ph);
                         if (i == 0 && jw[w] > 0) mbar_wait(pbar(w, P_OFREE), (jw[w] - 1) & 1);
                         tc_fence_after();
                         const uint32_t tO = tbase + w * PIPE_COLS;
@@ -256,7 +280,7 @@ attn_umma_kernel(const UParams P) {
                             for (int pg = 1; pg < TILE_PAGES; ++pg)
                                 if (pg < nvp) mma_ts(tO, tP + pg * 8, smem_desc_advance(vd, pg * HEAD_BLOCK), ID_PV, 1);
                             mma_commit(pbar(w, P_PVDONE + b));
-                            if (w == npipe - 1) mma_commit(bar(C::B_EMPTY + slot));
+                            if (w == npipe - 1) mma_commit(v_empty);
                         }
                         __syncwarp();
                     }
@@ -266,6 +290,55 @@ attn_umma_kernel(const UParams P) {
 #pragma unroll
             for (int w = 0; w < NP; ++w)
                 if (w < npipe) { g0[w] += n_tiles; jw[w]++; }
+        }
+    } else if (F8 && warp >= 2 + C::N_SOFTMAX / 32) {
+        // ================================ converter warps (FP8-KV) ================================
+        // Warp cw widens pages cw and cw + 2 of every landed e4m3 tile to fp16 (exact) into the K or the V
+        // operand slot: the same block image the bf16 path stages directly (swz_chunk_off(2, ...)).  The
+        // e4m3 block is 16 rows of 128 bytes, 16-byte chunks XOR-swizzled by (row & 7); a quarter warp
+        // takes one chunk column of 8 rows, which is conflict-free for the loads and for the stores.
+        // Rows of a partially filled last V page are written as zeros (pool memory may hold NaN codes).
+        const int cw = warp - (2 + C::N_SOFTMAX / 32);
+        uint32_t ct = 0;                                  // tiles of all items so far
+        for (int idx = item_begin; idx < item_end; ++idx) {
+            const WorkItem it = load_item(P.items, idx, P.seq_len);
+            const int n_tok = it.tok1 - it.tok0;
+            const int n_tiles = (n_tok + TILE_TOKENS - 1) / TILE_TOKENS;
+            for (int i = 0; i < n_tiles; ++i, ++ct) {
+                const int nv = min(TILE_TOKENS, n_tok - i * TILE_TOKENS);
+                const int np = (nv + PS - 1) / PS;
+#pragma unroll
+                for (int kv = 0; kv < 2; ++kv) {
+                    const uint32_t ld = 2 * ct + kv, slot = ld % NSLOT, ph = (ld / NSLOT) & 1;
+                    mbar_wait(bar(C::B_FULL + slot), ph);
+                    mbar_wait(bar(C::B_OPER + (kv ? O_VEMPTY : O_KEMPTY)), (ct & 1) ^ 1);
+                    const uint8_t *src = smem + C::RING_OFF + slot * C::RING_SLOT;
+                    uint8_t *dst = smem + C::OPER_OFF + kv * SLOT_BYTES;
+                    for (int pg = cw; pg < np; pg += 2) {
+                        const int valid = (kv && pg == np - 1 && (nv & (PS - 1))) ? (nv & (PS - 1)) : PS;
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4) {
+                            const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
+                            uint4 v = *reinterpret_cast<const uint4 *>(src + pg * (HEAD_BLOCK / 2) + row * 128 +
+                                                                       ((c8 ^ (row & 7)) << 4));
+                            uint4 a, b;
+                            e4m3x4_to_f16x4(v.x, a.x, a.y);
+                            e4m3x4_to_f16x4(v.y, a.z, a.w);
+                            e4m3x4_to_f16x4(v.z, b.x, b.y);
+                            e4m3x4_to_f16x4(v.w, b.z, b.w);
+                            if (row >= valid) a = b = make_uint4(0, 0, 0, 0);
+                            *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8)) = a;
+                            *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8 + 1)) = b;
+                        }
+                    }
+                    fence_async_smem();
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(bar(C::B_OPER + (kv ? O_VFULL : O_KFULL)));
+                        mbar_arrive(bar(C::B_EMPTY + slot));
+                    }
+                }
+            }
         }
     } else {
         // ================================ softmax warps ================================
@@ -295,6 +368,15 @@ attn_umma_kernel(const UParams P) {
                     const uint16_t *src =
                         P.q + ((size_t)item_qrow(qi, P.rowmap, lr, P.G) * P.Hq + qi.kvh * P.G + lr % P.G) * D + c * 8;
                     v[k] = *reinterpret_cast<const uint4 *>(src);
+                    if constexpr (F8) {       // bf16 -> fp16 (exact within fp16's range; beyond it saturates)
+                        uint32_t *u = reinterpret_cast<uint32_t *>(&v[k]);
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const float lo = fminf(fmaxf(__uint_as_float(u[e] << 16), -65504.f), 65504.f);
+                            const float hi = fminf(fmaxf(__uint_as_float(u[e] & 0xffff0000u), -65504.f), 65504.f);
+                            u[e] = pack_f16(lo, hi);
+                        }
+                    }
                 }
             }
 #pragma unroll
@@ -528,22 +610,30 @@ attn_umma_kernel(const UParams P) {
                     float a0, a1, c0, c1;
                     if (emulated_pair(2 * t)) ex2_poly2(x0, x1, a0, a1); else { a0 = ex2(x0); a1 = ex2(x1); }
                     if (emulated_pair(2 * t + 1)) ex2_poly2(y0, y1, c0, c1); else { c0 = ex2(y0); c1 = ex2(y1); }
-                    p[t] = pack_bf16(a0, a1);
-                    p[16 + t] = pack_bf16(c0, c1);
+                    p[t] = F8 ? pack_f16(a0, a1) : pack_bf16(a0, a1);
+                    p[16 + t] = F8 ? pack_f16(c0, c1) : pack_bf16(c0, c1);
                     // o is normalised by the sum of the ROUNDED weights the tensor core uses, so that
                     // o = sum(p v) / sum(p) stays a true weighted mean (a one-hot row returns V exactly
                     // even when the running max is stale and p is not a power of two); lse keeps the
                     // exact sum
                     fadd2(se0, se1, a0, a1);
                     fadd2(se2, se3, c0, c1);
+                    if constexpr (F8) {
+                        float r0, r1, r2, r3;
+                        unpack_f16(p[t], r0, r1);
+                        unpack_f16(p[16 + t], r2, r3);
+                        fadd2(sr0, sr1, r0, r1);
+                        fadd2(sr2, sr3, r2, r3);
+                    } else {
                     fadd2(sr0, sr1, __uint_as_float(p[t] << 16), __uint_as_float(p[t] & 0xffff0000u));
                     fadd2(sr2, sr3, __uint_as_float(p[16 + t] << 16), __uint_as_float(p[16 + t] & 0xffff0000u));
+                    }
                 }
                 l += (se0 + se1) + (se2 + se3);
                 lr += (sr0 + sr1) + (sr2 + sr3);
                 tmem_st32(tS, p);
                 tmem_wait_st();
-                if ((nv & (PS - 1)) && w == 0 && lg == 0) {
+                if (!F8 && (nv & (PS - 1)) && w == 0 && lg == 0) {
                     // the last staged page is partially filled: its tail rows hold whatever the pool
                     // held (possibly NaN patterns).  P is 0 there; make V 0 as well.  The warp of rows
                     // 0..31 does it (active in every item); the MMA thread issues pipe 0's P V, which
@@ -627,25 +717,25 @@ int attn_umma_grid(spork_ctx *c, int variant) {
     return c->num_sms * (variant == 1 ? Cfg<2, 1>::CTAS_PER_SM : Cfg<1, 1>::CTAS_PER_SM);
 }
 
-template <int NP, int SP>
+template <int NP, int SP, bool F8 = false>
 static int launch_np(spork_ctx *c, const UParams &p, int grid, bool programmatic, cudaStream_t st) {
-    constexpr uint32_t bit = 1u << (NP == 2 ? 1 : (SP == 2 ? 2 : 0));
+    constexpr uint32_t bit = 1u << (F8 ? 3 : (NP == 2 ? 1 : (SP == 2 ? 2 : 0)));
     if (!(c->smem_attr_done & bit)) {      // per handle (= per device), not per process
-        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        Cfg<NP, SP>::SMEM_BYTES));
+        SPORK_CUDA(cudaFuncSetAttribute(attn_umma_kernel<NP, SP, F8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Cfg<NP, SP, F8>::SMEM_BYTES));
         c->smem_attr_done |= bit;
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(Cfg<NP, SP>::N_THREADS);
-    cfg.dynamicSmemBytes = Cfg<NP, SP>::SMEM_BYTES;
+    cfg.blockDim = dim3(Cfg<NP, SP, F8>::N_THREADS);
+    cfg.dynamicSmemBytes = Cfg<NP, SP, F8>::SMEM_BYTES;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = programmatic ? 1 : 0;   // may start while the previous kernel drains
-    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP, SP>, p));
+    SPORK_CUDA(cudaLaunchKernelEx(&cfg, attn_umma_kernel<NP, SP, F8>, p));
     c->last_launches++;
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;
@@ -674,6 +764,7 @@ int launch_attn_umma(spork_ctx *c, const LayerIO &io, int np, bool programmatic,
     p.ws_o = (float *)c->ws_o.p;
     p.ws_lse = (float *)c->ws_lse.p;
     p.wait_prev = wait_prev ? 1 : 0;
+    if (c->cfg.dtype == SPORK_E4M3) return np == 1 ? launch_np<1, 1, true>(c, p, P.grid_umma, programmatic, st) : SPORK_ERR_INVALID;
     if (np == 1) return launch_np<1, 1>(c, p, P.grid_umma, programmatic, st);
     return P.variant2 == 2 ? launch_np<1, 2>(c, p, P.grid_umma2, programmatic, st)
                            : launch_np<2, 1>(c, p, P.grid_umma2, programmatic, st);

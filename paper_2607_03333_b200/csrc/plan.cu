@@ -375,7 +375,8 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     for (const Segment &s : segs) unique_tokens += s.tok1 - s.tok0;
 
     // ---- chunking --------------------------------------------------------------
-    const bool mma = c->cfg.dtype == SPORK_BF16 && c->cfg.head_dim == 128;
+    const bool f8 = c->cfg.dtype == SPORK_E4M3;     // tcgen05 kernel only (one-pipe shape), no mma.sync alternative
+    const bool mma = (c->cfg.dtype == SPORK_BF16 || f8) && c->cfg.head_dim == 128;
     const int grid_cap = mma ? attn_mma_grid(c) : c->num_sms * 4;
     // the generic (CUDA-core) kernel runs one warp per row and one CTA per item: short pieces and
     // row blocks of one warp each, so that even a tiny batch spreads over many SMs
@@ -383,7 +384,8 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
     int64_t total_cost = 0;
     for (Segment &s : segs) {
         const int rows = s.nq * G;
-        s.kind = !(mma && rows >= c->umma_min_rows) ? 0 : (rows > ROW_BLOCK_UMMA && c->many_row_variant ? 2 : 1);
+        s.kind = !(mma && (f8 || rows >= c->umma_min_rows)) ? 0
+                 : (!f8 && rows > ROW_BLOCK_UMMA && c->many_row_variant ? 2 : 1);
         s.row_block = s.kind == 0 ? (mma ? ROW_BLOCK : 4)
                                   : (s.kind == 2 && c->many_row_variant == 1 ? 2 : 1) * ROW_BLOCK_UMMA;
         int tiles = ceil_div(s.tok1 - s.tok0, TILE_TOKENS);

@@ -125,8 +125,9 @@ struct Plan {
 struct spork_ctx {
     spork_config cfg;
     int G;               // Hq / Hkv
-    int elt;             // bytes per element
-    int swizzled;        // bf16 && D % 64 == 0: 128B-swizzled page-head blocks
+    int elt;             // bytes per K / V element
+    int q_elt;           // bytes per Q element (= elt, except e4m3 KV: bf16 queries)
+    int swizzled;        // D * elt % 128 == 0 (bf16, e4m3): 128B-swizzled page-head blocks
     size_t head_block;   // bytes of one (page, kv head) block in one pool
     size_t page_bytes;   // bytes of one page in one pool
     int table_stride;    // int32 per block-table row (max_pages_per_seq rounded up to 4)
@@ -240,10 +241,12 @@ int launch_attn_mma(spork_ctx *c, const LayerIO &io, bool programmatic, cudaStre
 __host__ __device__ inline int swz_chunk_off(int nhalf, int r, int c) {
     return (((r >> 3) * nhalf + (c >> 3)) << 10) + ((r & 7) << 7) + (((c & 7) ^ (r & 7)) << 4);
 }
-// element offset (in elements) of (slot r, dim d) inside one (page, kv head) block
-__host__ __device__ inline int head_block_off(int swizzled, int D, int r, int d) {
+// element offset (in elements of `elt` bytes: 2 or 1 when swizzled) of (slot r, dim d) inside one
+// (page, kv head) block
+__host__ __device__ inline int head_block_off(int swizzled, int D, int elt, int r, int d) {
     if (!swizzled) return r * D + d;
-    return (swz_chunk_off(D >> 6, r, d >> 3) >> 1) + (d & 7);
+    const int per_chunk = 16 / elt;
+    return swz_chunk_off(D * elt >> 7, r, d / per_chunk) / elt + d % per_chunk;
 }
 
 #ifdef __CUDACC__

@@ -13,7 +13,7 @@ import numpy as np
 import oracle
 import synth
 
-OUT_TOL = {"f32": 1e-5, "bf16": 1e-2}
+OUT_TOL = {"f32": 1e-5, "bf16": 1e-2, "e4m3": 1e-2}    # e4m3 KV: DESIGN.md section 6
 LSE_RTOL = 1e-4
 
 
