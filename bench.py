@@ -42,7 +42,7 @@ import synth  # noqa: E402
 METRIC = "forked_decode_attn_unique_kv_bandwidth"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 L2_NOTE = "flushed between timed iterations (512 MiB write, then 256 MiB read so no dirty lines remain)"
-OUT_TOL = {"f32": 1e-5, "bf16": 1e-2}     # BASELINE.json north_star
+OUT_TOL = {"f32": 1e-5, "bf16": 1e-2, "e4m3": 1e-2}     # BASELINE.json north_star; e4m3 KV: DESIGN.md section 6
 LSE_RTOL = 1e-4
 
 
@@ -119,9 +119,8 @@ class ClockSampler:
 # workloads
 # ---------------------------------------------------------------------------
 def workload_name(cfg) -> str:
-    if cfg.cfg_no == 4:
-        return f"cfg4_qwen3_32b_verify_k{cfg.k_draft}"
-    return cfg.name
+    name = f"cfg4_qwen3_32b_verify_k{cfg.k_draft}" if cfg.cfg_no == 4 else cfg.name
+    return name + ("_e4m3kv" if cfg.dtype == "e4m3" else "")
 
 
 def pool_dims(wl, num_pages=None):
@@ -727,6 +726,8 @@ def run_single(env: Env, args):
     cfg = synth.CONFIGS[n]
     if n == 4:
         cfg = cfg.scaled(k_draft=args.k)
+    if args.kv == "e4m3":
+        cfg = cfg.scaled(dtype="e4m3")
     wl = synth.Workload(cfg)
     num_pages = (1 << 20) if (n == 5 and args.full_pool) else None
     spk, ids = build_spork(cfg, wl, num_pages, None, env.device)
@@ -780,6 +781,13 @@ def run_all(env: Env, args):
         spk.truncate(ids, wlk.total_len.astype(np.int32))
         per[f"cfg4_k{k}"] = measure_attn(env, spk, ids, cfgk, wlk)
     release_all(spk)
+    # ---- FP8-KV variant: configs 5 and 2 with an e4m3 cache (half the unique bytes) ----
+    for n in (5, 2):
+        cfg = synth.CONFIGS[n].scaled(dtype="e4m3")
+        wl = synth.Workload(cfg)
+        spk, ids = build_spork(cfg, wl, None, None, env.device)
+        per[f"cfg{n}_e4m3kv"] = measure_attn(env, spk, ids, cfg, wl)
+        release_all(spk)
     # ---- the append + decode loop on config 2, and config 1 ----
     per["loop_cfg2"] = measure_loop(env, synth.CFG2)
     per["cfg1"] = measure_cfg1(env)
@@ -931,6 +939,8 @@ def main():
     ap.add_argument("--min-rows", type=int, default=None,
                     help="planner knob: rows per KV head from which a segment runs on the tcgen05 kernel")
     ap.add_argument("--full-pool", action="store_true", help="config 5 on the 2^20-page pool")
+    ap.add_argument("--kv", default="bf16", choices=["bf16", "e4m3"],
+                    help="KV storage of configs 2-5: bf16 (BASELINE.json) or the FP8-KV variant (e4m3 K/V, bf16 Q)")
     args = ap.parse_args()
     if args.config == "d2":
         run_d2(args)

@@ -57,6 +57,7 @@ extern "C" {
 #define SPORK_ERR_SHARED (-6)       /* truncate would expose a shared partial page */
 #define SPORK_ERR_CUDA (-7)         /* a CUDA runtime call failed                  */
 #define SPORK_ERR_DEVICE (-8)       /* device-side consistency check tripped       */
+#define SPORK_ERR_STALE (-9)        /* a captured turn ran: call spork_turn_sync    */
 
 #define SPORK_F32 0
 #define SPORK_BF16 1
@@ -331,6 +332,45 @@ int spork_decode_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const i
 int spork_verify_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const int32_t *group_indptr,
                              const int32_t *seq_ids, const int32_t *q_indptr, const void *const *q,
                              float *const *out, float *const *lse, void *stream);
+
+/*
+ * One partial-token-accept turn without a host round trip, for CUDA-graph capture (SURVEY.md 8(f) NEXT-1:
+ * "end-to-end fork -> decode -> verify -> accept -> rollback step under one CUDA graph"; "in
+ * the same decode step (no separate verification pass)"; the decode loop of Algorithm 1 steps 4-5,
+ * PAPER.md:260-261).  The calls below enqueue ONLY kernel launches over buffers that do not move -- no
+ * host copy, no synchronisation, every decision (pages taken in request order: reading A-1; accept
+ * length; rollback) taken by kernels from the DEVICE lengths -- so the caller may capture any sequence
+ * of them, together with its own kernels, with cudaStreamBeginCapture (or torch.cuda.graph) on `stream`
+ * and replay the graph turn after turn:
+ *     spork_turn_append(t, 0, ...)   k_i draft tokens to every sequence (k_src, v_src: device,
+ *                                    [sum k_i][Hkv][D], ragged by q_indptr)
+ *     spork_turn_verify(t, ...)      as spork_verify_attn over the turn's batch (q [sum k_i][Hq][D])
+ *     spork_turn_accept(t, ...)      accept_len_i = leading positions with draft == target; the rejected
+ *                                    drafts are rolled back as spork_accept does; accept_len_dev: DEVICE
+ *                                    int32[n] or NULL
+ *     spork_turn_append(t, 1, ...)   one token to every sequence (k_src, v_src: [n][Hkv][D])
+ *     spork_turn_decode(t, ...)      as spork_decode_attn over the turn's batch (q [n][Hq][D])
+ * spork_turn_prepare (not capturable) fixes the batch: groups, sequences (each once, non-empty) and the
+ * number of drafts k_i = q_indptr[i+1] - q_indptr[i] in [1, 64] per sequence; it builds the two attention
+ * plans and uploads the descriptors.  The plans stay valid while sequences only grow (a turn nets
+ * accept_len + 1 tokens) and no other call changes the batch's sharing (fork / release / truncate of any
+ * sequence: the turn's calls then return SPORK_ERR_INVALID; prepare again).
+ * From the first turn call on the host's copy of the lengths is stale: every other state or attention
+ * call returns SPORK_ERR_STALE until spork_turn_sync (which synchronises `stream`, reads the lengths and
+ * the free-page count back, and returns SPORK_ERR_DEVICE if a turn ran out of pages or block-table row --
+ * such an append leaves the state untouched, as the host path does).  After a sync the graph can go on
+ * being replayed.  Errors: INVALID, INVALID_SEQ, STALE, CUDA.
+ */
+typedef struct spork_turn spork_turn;
+int spork_turn_prepare(spork_ctx *ctx, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
+                       const int32_t *q_indptr, void *stream, spork_turn **out);
+int spork_turn_append(spork_turn *t, int which, const void *k_src, const void *v_src, void *stream);
+int spork_turn_verify(spork_turn *t, const void *q, float *out, float *lse, void *stream);
+int spork_turn_accept(spork_turn *t, const int32_t *draft_tokens, const int32_t *target_tokens,
+                      int32_t *accept_len_dev, void *stream);
+int spork_turn_decode(spork_turn *t, const void *q, float *out, float *lse, void *stream);
+int spork_turn_sync(spork_turn *t, void *stream);
+int spork_turn_destroy(spork_turn *t);
 
 /*
  * Bench support: one read-only pass over `bytes` bytes at `buf` (device, 16-byte aligned), launched on

@@ -23,6 +23,7 @@ F32, BF16, E4M3 = 0, 1, 2
 PAGE_SIZE = 16
 
 OK = 0
+ERR_STALE = -9
 ERR_INVALID, ERR_OOM, ERR_NO_SLOT, ERR_TOO_LONG, ERR_INVALID_SEQ, ERR_SHARED, ERR_CUDA, ERR_DEVICE = (
     -1, -2, -3, -4, -5, -6, -7, -8)
 
@@ -35,6 +36,8 @@ ABI_SYMBOLS = [
     "spork_accept", "spork_confidence", "spork_set_timing", "spork_last_kernel_ms", "spork_set_tensor_path_min_rows", "spork_set_many_row_variant", "spork_set_stream_k", "spork_strerror",
     "spork_set_cascade_levels", "spork_layers", "spork_write_kv_layer", "spork_decode_attn_layers",
     "spork_verify_attn_layers", "spork_hbm_read_probe",
+    "spork_turn_prepare", "spork_turn_append", "spork_turn_verify", "spork_turn_accept", "spork_turn_decode",
+    "spork_turn_sync", "spork_turn_destroy",
 ]
 
 
@@ -106,6 +109,13 @@ def load(build_if_missing: bool = True):
         "spork_verify_attn_layers": ([P, I, I, P, P, P, P, P, P, P], I),
         "spork_last_kernel_ms": ([P, P, P], I),
         "spork_hbm_read_probe": ([P, P, C.c_size_t, P], I),
+        "spork_turn_prepare": ([P, I, P, P, P, P, P], I),
+        "spork_turn_append": ([P, I, P, P, P], I),
+        "spork_turn_verify": ([P, P, P, P, P], I),
+        "spork_turn_accept": ([P, P, P, P, P], I),
+        "spork_turn_decode": ([P, P, P, P, P], I),
+        "spork_turn_sync": ([P, P], I),
+        "spork_turn_destroy": ([P], I),
         "spork_strerror": ([I], C.c_char_p),
     }
     for name, (args, res) in sig.items():
@@ -278,6 +288,10 @@ class Spork:
         self._chk(rc, check)
         return out if check else (rc, out)
 
+    def turn(self, group_indptr, seq_ids, q_indptr) -> "Turn":
+        """Prepares a capturable partial-token-accept turn over this batch (see spork.h, spork_turn_*)."""
+        return Turn(self, group_indptr, seq_ids, q_indptr)
+
     # ---- attention ------------------------------------------------------------
     def decode_attn(self, group_indptr, seq_ids, q, out=None, lse=None, check: bool = True):
         """q: device tensor [n_seq][Hq][D] in the storage dtype (or numpy storage array).
@@ -441,3 +455,51 @@ class Spork:
 
     def synchronize(self):
         self.stream.synchronize()
+
+
+class Turn:
+    """A prepared turn: append drafts -> verify -> accept + rollback -> append one token -> decode, each
+    call nothing but kernel launches on the handle's stream over the DEVICE tensors it is given, so the
+    caller can capture them (torch.cuda.graph(..., stream=spk.stream)) and replay.  Argument marshalling
+    only; tensors must stay alive (and in place) for as long as a captured graph is replayed."""
+
+    def __init__(self, spk: Spork, group_indptr, seq_ids, q_indptr):
+        self.spk = spk
+        gi, s, qi = _i32(group_indptr), _i32(seq_ids), _i32(q_indptr)
+        self.n, self.rows = len(s), int(qi[-1])
+        h = C.c_void_p()
+        spk._chk(spk.lib.spork_turn_prepare(spk._h, len(gi) - 1, _p(gi), _p(s), _p(qi), spk._st, C.byref(h)))
+        self._t = h
+
+    def append(self, which: int, k, v):
+        """which = 0: the k_i drafts of every sequence ([sum k][Hkv][D]); 1: one token each ([n][Hkv][D])."""
+        self.spk._chk(self.spk.lib.spork_turn_append(self._t, int(which), C.c_void_p(k.data_ptr()),
+                                                      C.c_void_p(v.data_ptr()), self.spk._st))
+
+    def verify(self, q, out, lse):
+        self.spk._chk(self.spk.lib.spork_turn_verify(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                      C.c_void_p(lse.data_ptr()), self.spk._st))
+
+    def accept(self, draft_tokens, target_tokens, accept_len=None):
+        a = C.c_void_p(accept_len.data_ptr()) if accept_len is not None else None
+        self.spk._chk(self.spk.lib.spork_turn_accept(self._t, C.c_void_p(draft_tokens.data_ptr()),
+                                                      C.c_void_p(target_tokens.data_ptr()), a, self.spk._st))
+
+    def decode(self, q, out, lse):
+        self.spk._chk(self.spk.lib.spork_turn_decode(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                      C.c_void_p(lse.data_ptr()), self.spk._st))
+
+    def sync(self, check: bool = True) -> int:
+        """Host mirror of the lengths <- device (synchronises); the other Spork calls work again."""
+        return self.spk._chk(self.spk.lib.spork_turn_sync(self._t, self.spk._st), check)
+
+    def close(self):
+        if getattr(self, "_t", None):
+            self.spk.lib.spork_turn_destroy(self._t)
+            self._t = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

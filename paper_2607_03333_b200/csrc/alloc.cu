@@ -118,14 +118,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) free_compact_kernel(
     }
 }
 
-// ---- append ----------------------------------------------------------------
-struct AppendDesc {
-    int32_t seq, old_len, n_tok, tok_off;
-    int32_t free_off;   // index into free_list of this request's first new page
-    int32_t n_new;      // pages this request allocates
-    int32_t final_len;  // >= 0: this request writes len[seq] (last request of the sequence)
-    int32_t pad;
-};
+// ---- append (AppendDesc: spork_internal.h) -----------------------------------
 
 __global__ void append_assign_kernel(const AppendDesc *__restrict__ descs, int n,
                                      const int32_t *__restrict__ free_list, int32_t *refcount,
@@ -390,6 +383,18 @@ int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st) {
     return need <= c->free_lb ? SPORK_OK : SPORK_ERR_OOM;
 }
 
+// the one-kernel append over descriptors that are already on the device (spork_append's fast path; turn.cu)
+int launch_append_small(spork_ctx *c, const AppendDesc *d_descs, int n, int need, const void *k_src,
+                        const void *v_src, cudaStream_t st) {
+    append_small_kernel<<<n, 128, 0, st>>>(
+        d_descs, c->d_free_list, c->d_refcount, c->d_table, c->table_stride, c->d_len, c->d_counters, need,
+        (const uint4 *)k_src, (const uint4 *)v_src, (uint8_t *)c->k_pool, (uint8_t *)c->v_pool,
+        c->cfg.num_kv_heads, c->cfg.head_dim * c->elt / 16, c->swizzled, c->head_block);
+    c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
 // `need` lowest free page ids, ascending, at d_free_list[*off ..).  The list of one scan is cached: as long
 // as no page has been FREED since (release / truncate / accept invalidate it), the ids behind the ones
 // already handed out are still the lowest free ones, so an append-only phase (the decode loop) scans
@@ -419,6 +424,7 @@ int take_free(spork_ctx *c, int need, cudaStream_t st, int *off) {
 extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const int32_t *n_tokens,
                             const void *k_src, const void *v_src, void *stream) {
     if (!c || n < 0 || (n > 0 && (!seq_ids || !n_tokens))) return SPORK_ERR_INVALID;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     cudaStream_t st = (cudaStream_t)stream;
     c->last_launches = 0;
     if (n == 0) return SPORK_OK;
@@ -479,12 +485,8 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
     rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
     if (rc != SPORK_OK) return rc;
     if (small) {
-        append_small_kernel<<<n, 128, 0, st>>>(
-            (const AppendDesc *)slot->d, c->d_free_list, c->d_refcount, c->d_table, c->table_stride, c->d_len,
-            c->d_counters, (int)need, (const uint4 *)k_src, (const uint4 *)v_src, (uint8_t *)c->k_pool,
-            (uint8_t *)c->v_pool, c->cfg.num_kv_heads, c->cfg.head_dim * c->elt / 16, c->swizzled, c->head_block);
-        c->last_launches++;
-        SPORK_CUDA(cudaGetLastError());
+        rc = launch_append_small(c, (const AppendDesc *)slot->d, n, (int)need, k_src, v_src, st);
+        if (rc != SPORK_OK) return rc;
         c->free_lb -= need;
         c->len_epoch++;
         return stage_done(c, slot, st);
@@ -515,6 +517,7 @@ extern "C" int spork_write_kv_layer(spork_ctx *c, int layer, int n, const int32_
                                     const int32_t *n_tokens, const void *k_src, const void *v_src, void *stream) {
     if (!c || n < 0 || (n > 0 && (!seq_ids || !n_tokens))) return SPORK_ERR_INVALID;
     if (layer < 0 || layer > (int)c->layer_k.size()) return SPORK_ERR_INVALID;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     cudaStream_t st = (cudaStream_t)stream;
     c->last_launches = 0;
     if (n == 0) return SPORK_OK;
@@ -554,6 +557,7 @@ extern "C" int spork_write_kv_layer(spork_ctx *c, int layer, int n, const int32_
 extern "C" int spork_fork(spork_ctx *c, int n, const int32_t *parent_ids, int32_t *child_ids_out,
                           void *stream) {
     if (!c || n < 0 || (n > 0 && (!parent_ids || !child_ids_out))) return SPORK_ERR_INVALID;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     cudaStream_t st = (cudaStream_t)stream;
     c->last_launches = 0;
     if (n == 0) return SPORK_OK;
@@ -641,6 +645,7 @@ static int drop_common(spork_ctx *c, int n, const int32_t *seq_ids, const int32_
                        cudaStream_t st) {
     // new_len == nullptr: release.  Errors are reported for the first offending request in array
     // order; a possibly-shared kept tail page BEFORE that request is resolved on the device first.
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     for (int i = 0; i < n; ++i) {
         int s = seq_ids[i];
         if (s >= 0 && s < c->cfg.max_seqs) c->h_scratch[s] = 0;
@@ -792,6 +797,7 @@ extern "C" int spork_accept(spork_ctx *c, int n, const int32_t *seq_ids, const i
     if (n == 0) return SPORK_OK;
     if (!seq_ids || !q_indptr || !draft_tokens || !target_tokens || !accept_len_out || q_indptr[0] != 0)
         return SPORK_ERR_INVALID;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     cudaStream_t st = (cudaStream_t)stream;
     for (int i = 0; i < n; ++i) {
         const int s = seq_ids[i], k = q_indptr[i + 1] - q_indptr[i];

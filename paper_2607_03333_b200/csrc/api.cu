@@ -81,6 +81,7 @@ extern "C" const char *spork_strerror(int code) {
         case SPORK_ERR_SHARED: return "truncate into a shared partial page";
         case SPORK_ERR_CUDA: return "CUDA runtime error";
         case SPORK_ERR_DEVICE: return "device-side consistency check failed";
+        case SPORK_ERR_STALE: return "host lengths are stale after a captured turn: call spork_turn_sync";
         default: return "unknown spork error";
     }
 }
@@ -278,6 +279,7 @@ __global__ void read_kv_kernel(const T *__restrict__ kpool, const T *__restrict_
 extern "C" int spork_read_kv(spork_ctx *c, int32_t seq, int32_t t0, int32_t n, void *k_out,
                              void *v_out) {
     if (!c || seq < 0 || seq >= c->cfg.max_seqs || !c->h_live[seq]) return SPORK_ERR_INVALID_SEQ;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     if (t0 < 0 || n < 0 || t0 + n > c->h_len[seq] || (n > 0 && (!k_out || !v_out)))
         return SPORK_ERR_INVALID;
     if (n == 0) return SPORK_OK;

@@ -29,9 +29,22 @@ static int launch_layer(spork_ctx *c, const LayerIO &io, bool chained, cudaStrea
     return rc;
 }
 
+namespace spork {
+int launch_planned(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
+    Plan &P = c->plan;
+    if (!P.valid) return SPORK_ERR_INVALID;
+    if (P.n_qrows == 0) return SPORK_OK;
+    if (!io.q || !io.out || !io.lse) return SPORK_ERR_INVALID;
+    int rc = launch_layer(c, io, false, st);
+    if (rc == SPORK_OK) rc = launch_merge(c, io, st);
+    return rc;
+}
+}  // namespace spork
+
 static int attn_layers(spork_ctx *c, int n_layers, int n_groups, const int32_t *group_indptr,
                        const int32_t *seq_ids, const int32_t *q_indptr, const LayerIO *io, cudaStream_t st) {
     c->last_launches = 0;
+    if (c->mirror_stale) return SPORK_ERR_STALE;
     int rc = build_plan(c, n_groups, group_indptr, seq_ids, q_indptr, st);
     if (rc != SPORK_OK) return rc;
     Plan &P = c->plan;

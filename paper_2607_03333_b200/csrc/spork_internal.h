@@ -61,6 +61,16 @@ struct QRowDesc {
 static_assert(sizeof(QRowDesc) == 8 && sizeof(RowRef) == 8, "merge descriptor layout");
 constexpr int MAX_ROW_REFS = 8;     // deepest cascade: 7 shared levels + the private tail
 
+// One append request as the append kernels read it (built on the host by spork_append, on the device by
+// the captured turn: turn.cu)
+struct AppendDesc {
+    int32_t seq, old_len, n_tok, tok_off;
+    int32_t free_off;   // index into free_list of this request's first new page
+    int32_t n_new;      // pages this request allocates
+    int32_t final_len;  // >= 0: this request writes len[seq] (last request of the sequence)
+    int32_t pad;
+};
+
 // Host lineage of a sequence: which incarnation allocated each of its pages, run-length encoded.
 // Pages [r[i-1].end, r[i].end) were allocated by incarnation r[i].uid (a fresh uid is drawn at
 // seq_create, at fork (for the child) and at truncate).  Two sequences hold the same physical page at
@@ -155,6 +165,7 @@ struct spork_ctx {
     std::vector<uint64_t> h_uid;         // current incarnation of the slot
     uint64_t next_uid = 1;
     int64_t free_lb;                     // lower bound on free pages
+    bool mirror_stale = false;           // a captured turn ran: lengths live on the device only until spork_turn_sync
     bool fl_valid = false;               // d_free_list[fl_pos, fl_n) are still the lowest free ids (see take_free)
     int fl_pos = 0, fl_n = 0;
     int n_live;
@@ -206,6 +217,9 @@ int devbuf_reserve(DevBuf *b, size_t bytes, cudaStream_t st);
 int launch_free_scan(spork_ctx *c, int need, cudaStream_t st);  // fills d_free_list[0..need)
 int ensure_pages(spork_ctx *c, int64_t need, cudaStream_t st);  // OOM check (may sync)
 int take_free(spork_ctx *c, int need, cudaStream_t st, int *off);  // ids at d_free_list[*off, *off + need)
+int launch_append_small(spork_ctx *c, const AppendDesc *d_descs, int n, int need, const void *k_src,
+                        const void *v_src, cudaStream_t st);
+
 
 // plan.cu
 int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const int32_t *seq_ids,
@@ -225,6 +239,8 @@ struct LayerIO {
     float *out, *lse;
 };
 int launch_attn_simt(spork_ctx *c, const LayerIO &io, cudaStream_t st);
+// attn_api.cu: attention + merge kernels of the plan that is in c->plan, one layer
+int launch_planned(spork_ctx *c, const LayerIO &io, cudaStream_t st);
 int launch_merge(spork_ctx *c, const LayerIO &io, cudaStream_t st);
 int attn_mma_grid(spork_ctx *c);
 int launch_attn_umma(spork_ctx *c, const LayerIO &io, int np, bool programmatic, bool wait_prev, cudaStream_t st);
