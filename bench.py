@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line per run (the driver's contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|churn|loop|layers|d2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|churn|loop|turn|d2] [--kv bf16|e4m3]
                     [--k 4|8|16] [--impl reference]
 
 A step = one pass of the hot path over one batch of synthetic input:
@@ -11,6 +11,8 @@ A step = one pass of the hot path over one batch of synthetic input:
   churn          one spork_fork of 10,000 children + one spork_release of them (config 5, 2^20-page pool)
   loop           spork_append of one token to every sequence + spork_decode_attn (Alg. 1 step 5,
                  PAPER.md:261; the paper's decode loop), on config 2
+  turn           one partial-token-accept turn of config 4's batch (append k drafts, verify, accept +
+                 rollback, append one token, decode) captured in ONE CUDA graph and replayed (spork_turn_*)
   d2             one spork_confidence call: Eq. 2 over 256 probe spans of Qwen3-vocabulary logits
 Default (`--config all`): the headline is the LARGEST single-GPU decode config of BASELINE.json
 (config 5: 16 fork groups of 8, prefix 32768, 1.59 GB of unique KV); the same JSON line carries a
@@ -691,6 +693,92 @@ def measure_loop(env: Env, cfg, n_steps=None):
             "final_mean_len": float(np.mean(L_end))}
 
 
+def measure_turn(env: Env, k=16, n_turns=30):
+    """config 4's batch, one partial-token-accept turn per step, captured in ONE CUDA graph and replayed
+    (spork_turn_*: no host round trip): append k drafts -> verify -> accept + rollback -> append 1 token ->
+    decode.  Random accept lengths (uniform in 0..k), so sequences grow by k/2 + 1 tokens per turn."""
+    torch, args = env.torch, env.args
+    cfg = synth.CFG4.scaled(k_draft=0)
+    wl = synth.Workload(cfg)
+    grow = (n_turns + max(args.warmup, 3) + 4) * (k + 1) + k
+    spk, ids = build_spork(cfg, wl, device=env.device, extra_pages_per_seq=grow // 16 + 2,
+                           num_pages=pool_dims(wl)[0] + cfg.n_seqs * (grow // 16 + 2))
+    st = spk.stream
+    n, tot = cfg.n_seqs, cfg.n_seqs * k
+    ks = np.full(n, k, np.int64)
+    qi = np.concatenate([[0], np.cumsum(ks)]).astype(np.int32)
+    r = synth.rng(cfg.cfg_no, synth.T_MISC, 99)
+    f = lambda *shape: spk._dev(synth.to_storage(r.standard_normal(shape, dtype=np.float32), cfg.dtype))
+    kd, vd, qv = f(tot, cfg.Hkv, cfg.D), f(tot, cfg.Hkv, cfg.D), f(tot, cfg.Hq, cfg.D)
+    k1, v1, qd = f(n, cfg.Hkv, cfg.D), f(n, cfg.Hkv, cfg.D), f(n, cfg.Hq, cfg.D)
+    draft_np = r.integers(0, 50000, size=tot).astype(np.int32)
+    target_np = draft_np.copy()
+    acc_want = r.integers(0, k + 1, size=n)
+    for i in range(n):
+        target_np[qi[i] + acc_want[i]:qi[i + 1]] += 1
+    draft, target = spk._dev(draft_np), spk._dev(target_np)
+    dev = env.device
+    out_v = torch.empty((tot, cfg.Hq, cfg.D), dtype=torch.float32, device=dev)
+    lse_v = torch.empty((tot, cfg.Hq), dtype=torch.float32, device=dev)
+    out_d = torch.empty((n, cfg.Hq, cfg.D), dtype=torch.float32, device=dev)
+    lse_d = torch.empty((n, cfg.Hq), dtype=torch.float32, device=dev)
+    acc = torch.zeros(n, dtype=torch.int32, device=dev)
+    turn = spk.turn(wl.group_indptr(), ids, qi)
+    launches = [0]
+
+    def enqueue():
+        turn.append(0, kd, vd)
+        a = spk.last_launches()
+        turn.verify(qv, out_v, lse_v)
+        b = spk.last_launches()
+        turn.accept(draft, target, acc)
+        c = spk.last_launches()
+        turn.append(1, k1, v1)
+        d = spk.last_launches()
+        turn.decode(qd, out_d, lse_d)
+        launches[0] = a + b + c + d + spk.last_launches()
+
+    enqueue()                                   # eager warm-up turn
+    spk.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        enqueue()
+    with torch.cuda.stream(st):
+        for _ in range(max(args.warmup, 3)):
+            env.flush_l2(st)
+            g.replay()
+    env.barrier()
+    evs = []
+    with torch.cuda.stream(st):
+        for _ in range(n_turns):
+            env.flush_l2(st)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(st)
+            g.replay()
+            b.record(st)
+            evs.append((a, b))
+    torch.cuda.synchronize()
+    ms_turn = env.mx(float(np.mean([a.elapsed_time(b) for a, b in evs])))
+    # the same turn issued call by call (eager launches, no graph), wall clock per turn back to back
+    t0 = time.perf_counter()
+    for _ in range(4):
+        enqueue()
+    spk.synchronize()
+    eager = (time.perf_counter() - t0) / 4
+    rc = turn.sync(check=False)
+    assert rc == 0 and np.array_equal(acc.cpu().numpy(), acc_want), "turn state went wrong"
+    lens = np.array([spk.export(int(s))[0] for s in ids])
+    turn.close()
+    spk.close()
+    return {"workload": f"cfg4_turn_k{k}_cuda_graph", "turn_us": ms_turn * 1e3, "ms_per_step": ms_turn,
+            "us_per_step": ms_turn * 1e3, "turns": n_turns, "kernels_per_turn": launches[0],
+            "eager_wall_us_per_turn": eager * 1e6, "mean_accept_len": float(acc_want.mean()),
+            "value": env.world * cfg.n_seqs * (k + 1) / (ms_turn * 1e-3), "unit": "query rows/s",
+            "note": "one graph replay = append k drafts, verify, accept + rollback, append 1 token, decode; "
+                    "L2 flushed before every replay; no host round trip inside the turn",
+            "final_mean_len": float(lens.mean())}
+
+
 def release_all(spk):
     spk.close()
     gc.collect()
@@ -790,6 +878,7 @@ def run_all(env: Env, args):
         release_all(spk)
     # ---- the append + decode loop on config 2, and config 1 ----
     per["loop_cfg2"] = measure_loop(env, synth.CFG2)
+    per["turn_cfg4_k16"] = measure_turn(env, 16)
     per["cfg1"] = measure_cfg1(env)
     line = headline_line(env, head, cfg5)
     line["config"]["pool_pages"] = NP5
@@ -927,7 +1016,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="all", choices=["all", "1", "2", "3", "4", "5", "churn", "loop", "d2"])
+    ap.add_argument("--config", default="all",
+                    choices=["all", "1", "2", "3", "4", "5", "churn", "loop", "turn", "d2"])
     ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-groups", type=int, default=0,
@@ -949,7 +1039,7 @@ def main():
         # the oracle on the host cores, on this arm's headline workload (config 5 unless --config says otherwise)
         if int(os.environ.get("RANK", "0")) != 0:
             return
-        n = 5 if args.config in ("all", "churn", "loop") else int(args.config)
+        n = 5 if args.config in ("all", "churn", "loop", "turn") else int(args.config)
         cfg = synth.CONFIGS[n]
         if n == 4:
             cfg = cfg.scaled(k_draft=args.k)
@@ -971,6 +1061,12 @@ def main():
         rec = measure_loop(env, synth.CFG2)
         line = dict(rec, metric="append_decode_loop_us_per_step", n_gpus=env.world, higher_is_better=True,
                     scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic",
+                    config={"workload": rec["workload"], "l2": L2_NOTE})
+    elif args.config == "turn":
+        rec = measure_turn(env, args.k if args.k else 16)
+        line = dict(rec, metric="partial_token_accept_turn_us", n_gpus=env.world, higher_is_better=False,
+                    scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic", steps=rec["turns"],
+                    warmup=max(args.warmup, 3), gpu_launches=rec["kernels_per_turn"] * rec["turns"],
                     config={"workload": rec["workload"], "l2": L2_NOTE})
     elif args.config == "1":
         rec = measure_cfg1(env)
