@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- one JSON line per run (the driver's contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|churn|loop|turn|d2] [--kv bf16|e4m3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config all|1|2|3|4|5|churn|loop|turn|successive|layers|d2] [--kv bf16|e4m3]
                     [--k 4|8|16] [--impl reference]
 
 A step = one pass of the hot path over one batch of synthetic input:
@@ -11,6 +11,8 @@ A step = one pass of the hot path over one batch of synthetic input:
   churn          one spork_fork of 10,000 children + one spork_release of them (config 5, 2^20-page pool)
   loop           spork_append of one token to every sequence + spork_decode_attn (Alg. 1 step 5,
                  PAPER.md:261; the paper's decode loop), on config 2
+  successive     config 3's shape with probes forked at successive CoT positions: multi-level vs one-level cascade
+  layers         config 2's batch over 36 layers: one plan, 36 chained (attention, merge) launches
   turn           one partial-token-accept turn of config 4's batch (append k drafts, verify, accept +
                  rollback, append one token, decode) captured in ONE CUDA graph and replayed (spork_turn_*)
   d2             one spork_confidence call: Eq. 2 over 256 probe spans of Qwen3-vocabulary logits
@@ -693,6 +695,101 @@ def measure_loop(env: Env, cfg, n_steps=None):
             "final_mean_len": float(np.mean(L_end))}
 
 
+def measure_successive(env: Env):
+    """Successive probes (Algorithm 1 steps 4-6): config 3's shape,
+    32 mains, 3 probes forked after 500 / 1000 / 1500 further CoT tokens.  The multi-level cascade reads
+    every shared run once; with one level (the round-1 planner) everything beyond the first fork point is
+    read once per member.  Same kernels, same outputs: only the plan differs."""
+    args = env.args
+    cfg = synth.CFG3
+    wl = synth.SuccessiveWorkload(cfg, 500)
+    per_seq = int(wl.total_len.max()) // 16 + 4
+    npg = int(sum(int(x) // 16 + 2 for x in wl.total_len)) + 1024
+    import paper_2607_03333_b200 as sp
+    spk = sp.Spork(cfg.dtype, cfg.Hq, cfg.Hkv, cfg.D, npg, cfg.n_seqs + 8, per_seq, cfg.scale, device=env.device)
+    ids = synth.build_state_successive(spk, wl)
+    spk.synchronize()
+    st = spk.stream
+    gi = wl.group_indptr()
+    q_dev = spk._dev(wl.q_all())
+    out, lse = spk.decode_attn(gi, ids, q_dev)
+    rec = {"workload": "cfg3_successive_probes_500_1000_1500", "dtype": cfg.dtype,
+           "nested_unique_tokens": wl.unique_tokens(), "single_level_tokens": wl.single_level_tokens(),
+           "naive_tokens": wl.naive_tokens()}
+    for name, lv in (("multi_level", 7), ("single_level", 1)):
+        spk.set_cascade_levels(lv)
+
+        def step():
+            spk.decode_attn(gi, ids, q_dev, out, lse)
+
+        for _ in range(max(args.warmup, 3)):
+            env.flush_l2(st)
+            step()
+        env.barrier()
+        ms = env.mx(sum(env.timed(st, step, args.steps))) / args.steps
+        info = spk.last_plan()
+        by = info["unique_tokens"] * cfg.token_bytes
+        rec[name] = {"us_per_step": ms * 1e3, "plan_tokens_read": info["unique_tokens"], "bytes_read_model": by,
+                     "GBps": by / (ms * 1e-3) / 1e9, "n_levels": info["n_levels"], "n_items": info["n_items"]}
+    assert rec["multi_level"]["plan_tokens_read"] == wl.unique_tokens()
+    assert rec["single_level"]["plan_tokens_read"] == wl.single_level_tokens()
+    ub = wl.unique_tokens() * cfg.token_bytes
+    ms = rec["multi_level"]["us_per_step"] * 1e-3
+    rec.update({"ms_per_step": ms, "us_per_step": ms * 1e3, "unique_kv_bytes": ub,
+                "value": aggregate_value(ub, ms, env.world), "unit": "GB/s", "frac_of_8TBps": ub / (ms * 1e-3) / 1e9 / 8000.0,
+                "speedup_vs_single_level": rec["single_level"]["us_per_step"] / rec["multi_level"]["us_per_step"]})
+    if env.rank == 0 and not args.no_cpu_baseline:
+        rec["parity"] = parity_spot_check(cfg, wl, out.cpu().numpy(), lse.cpu().numpy())
+    spk.close()
+    return rec
+
+
+def measure_layers(env: Env, n_layers=36):
+    """Multi-layer step: config 2's batch over the 36 layers of Qwen3-4B:
+    ONE plan, 36 x (attention, merge) launches chained programmatically.  Layers 1.. hold copies of layer
+    0's K/V (the values do not matter for the time)."""
+    torch, args = env.torch, env.args
+    cfg = synth.CFG2
+    wl = synth.Workload(cfg)
+    spk, ids = build_spork(cfg, wl, device=env.device)
+    spk.layers(n_layers)
+    with torch.cuda.stream(spk.stream):
+        for l in range(1, n_layers):
+            spk.k_pools[l].copy_(spk.k_pool)
+            spk.v_pools[l].copy_(spk.v_pool)
+    st = spk.stream
+    gi = wl.group_indptr()
+    q0 = spk._dev(wl.q_all())
+    qs = [q0] + [q0.clone() for _ in range(n_layers - 1)]
+    outs = [torch.empty((cfg.n_seqs, cfg.Hq, cfg.D), dtype=torch.float32, device=env.device) for _ in range(n_layers)]
+    lses = [torch.empty((cfg.n_seqs, cfg.Hq), dtype=torch.float32, device=env.device) for _ in range(n_layers)]
+
+    def step():
+        spk.attn_layers(gi, ids, qs, outs, lses)
+
+    def single():
+        spk.decode_attn(gi, ids, q0, outs[0], lses[0])
+
+    for _ in range(max(args.warmup, 3)):
+        env.flush_l2(st)
+        step()
+    env.barrier()
+    n = max(5, args.steps // 2)
+    ms = env.mx(sum(env.timed(st, step, n))) / n
+    single()
+    ms1 = env.mx(sum(env.timed(st, single, args.steps))) / args.steps
+    launches = spk.last_plan()["launches"]
+    ub = wl.unique_kv_bytes()
+    same = bool(torch.equal(outs[0], outs[n_layers - 1]))     # identical pools and q: identical results
+    spk.close()
+    return {"workload": f"cfg2_x{n_layers}_layers", "layers": n_layers, "ms_per_step": ms, "us_per_step": ms * 1e3,
+            "us_per_layer": ms * 1e3 / n_layers, "single_layer_call_us": ms1 * 1e3,
+            "value": aggregate_value(ub * n_layers, ms, env.world), "unit": "GB/s",
+            "frac_of_8TBps": ub * n_layers / (ms * 1e-3) / 1e9 / 8000.0, "unique_kv_bytes_per_layer": ub,
+            "last_layer_equals_first": same, "dtype": cfg.dtype,
+            "note": "K/V of 36 layers = 14 GB: nothing of a layer survives in L2 until its next use"}
+
+
 def measure_turn(env: Env, k=16, n_turns=30):
     """config 4's batch, one partial-token-accept turn per step, captured in ONE CUDA graph and replayed
     (spork_turn_*: no host round trip): append k drafts -> verify -> accept + rollback -> append 1 token ->
@@ -879,6 +976,8 @@ def run_all(env: Env, args):
     # ---- the append + decode loop on config 2, and config 1 ----
     per["loop_cfg2"] = measure_loop(env, synth.CFG2)
     per["turn_cfg4_k16"] = measure_turn(env, 16)
+    per["successive_cfg3"] = measure_successive(env)
+    per["layers_cfg2_x36"] = measure_layers(env, 36)
     per["cfg1"] = measure_cfg1(env)
     line = headline_line(env, head, cfg5)
     line["config"]["pool_pages"] = NP5
@@ -1017,7 +1116,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="all",
-                    choices=["all", "1", "2", "3", "4", "5", "churn", "loop", "turn", "d2"])
+                    choices=["all", "1", "2", "3", "4", "5", "churn", "loop", "turn", "successive", "layers", "d2"])
     ap.add_argument("--k", type=int, default=8, help="drafts per sequence for config 4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-groups", type=int, default=0,
@@ -1039,7 +1138,7 @@ def main():
         # the oracle on the host cores, on this arm's headline workload (config 5 unless --config says otherwise)
         if int(os.environ.get("RANK", "0")) != 0:
             return
-        n = 5 if args.config in ("all", "churn", "loop", "turn") else int(args.config)
+        n = 5 if args.config in ("all", "churn", "loop", "turn", "successive", "layers") else int(args.config)
         cfg = synth.CONFIGS[n]
         if n == 4:
             cfg = cfg.scaled(k_draft=args.k)
@@ -1061,6 +1160,11 @@ def main():
         rec = measure_loop(env, synth.CFG2)
         line = dict(rec, metric="append_decode_loop_us_per_step", n_gpus=env.world, higher_is_better=True,
                     scaling="weak", vs_baseline=None, dtype="bf16", data="synthetic",
+                    config={"workload": rec["workload"], "l2": L2_NOTE})
+    elif args.config in ("successive", "layers"):
+        rec = measure_successive(env) if args.config == "successive" else measure_layers(env, 36)
+        line = dict(rec, metric=METRIC, n_gpus=env.world, steps=args.steps, warmup=max(args.warmup, 3),
+                    higher_is_better=True, scaling="weak", vs_baseline=None, data="synthetic",
                     config={"workload": rec["workload"], "l2": L2_NOTE})
     elif args.config == "turn":
         rec = measure_turn(env, args.k if args.k else 16)
