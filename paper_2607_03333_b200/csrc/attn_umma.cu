@@ -59,8 +59,8 @@ __host__ __device__ constexpr bool emulated_pair(int j) { return (j * EMU_NUM) %
 //           4 per SM sub-partition instead of 2) for items whose time is the softmax's, not HBM's:
 //           4-slot ring, the row max and the row sums are exchanged through shared memory
 //   F8 (NP = SP = 1): the FP8-KV variant (e4m3 K/V bytes, bf16 Q).  The bulk copies land 8 KiB e4m3 tiles
-//           in a 6-slot ring; two converter warps widen them (exactly) to fp16 into ONE K operand slot and
-//           ONE V operand slot in the same swizzled image the bf16 path stages directly, Q is converted
+//           in a 6-slot ring; two converter warps (one for K, one for V) widen them (exactly) to fp16 into ONE
+//           K operand slot and ONE V operand slot in the same swizzled image the bf16 path stages directly, Q is converted
 //           bf16 -> fp16 when it is staged, P is packed as fp16: the MMAs run in kind::f16 with fp16
 //           operands, everything downstream of the operands is the bf16 kernel.
 template <int NP, int SP, bool F8 = false>
@@ -128,7 +128,7 @@ attn_umma_kernel(const UParams P) {
         if (sbase & 1023u) __trap();   // the 128-byte swizzle is a function of the smem address
         for (int s = 0; s < NSLOT; ++s) {
             mbar_init(bar(C::B_FULL + s), 1);
-            mbar_init(bar(C::B_EMPTY + s), F8 ? 2 : 1);
+            mbar_init(bar(C::B_EMPTY + s), 1);
         }
         for (int w = 0; w < NP; ++w) {
             for (int b = 0; b < 2; ++b) {
@@ -140,8 +140,8 @@ attn_umma_kernel(const UParams P) {
         }
         mbar_init(bar(C::B_QFULL), 1);
         if constexpr (F8) {
-            mbar_init(bar(C::B_OPER + O_KFULL), 2);     // one arrival per converter warp
-            mbar_init(bar(C::B_OPER + O_VFULL), 2);
+            mbar_init(bar(C::B_OPER + O_KFULL), 1);     // the K converter warp
+            mbar_init(bar(C::B_OPER + O_VFULL), 1);     // the V converter warp
             mbar_init(bar(C::B_OPER + O_KEMPTY), 1);    // tcgen05.commit
             mbar_init(bar(C::B_OPER + O_VEMPTY), 1);
         }
@@ -293,12 +293,19 @@ attn_umma_kernel(const UParams P) {
         }
     } else if (F8 && warp >= 2 + C::N_SOFTMAX / 32) {
         // ================================ converter warps (FP8-KV) ================================
-        // Warp cw widens pages cw and cw + 2 of every landed e4m3 tile to fp16 (exact) into the K or the V
-        // operand slot: the same block image the bf16 path stages directly (swz_chunk_off(2, ...)).  The
-        // e4m3 block is 16 rows of 128 bytes, 16-byte chunks XOR-swizzled by (row & 7); a quarter warp
+        // Warp 0 of the two widens every landed K tile, warp 1 every V tile, e4m3 -> fp16 (exact), into the K
+        // / V operand slot: the same block image the bf16 path stages directly (swz_chunk_off(2, ...)).
+        // The e4m3 block is 16 rows of 128 bytes, 16-byte chunks XOR-swizzled by (row & 7); a quarter warp
         // takes one chunk column of 8 rows, which is conflict-free for the loads and for the stores.
         // Rows of a partially filled last V page are written as zeros (pool memory may hold NaN codes).
-        const int cw = warp - (2 + C::N_SOFTMAX / 32);
+        // A tile's 16 loads are issued before the warp waits for its operand slot (the landing slot is
+        // released as soon as they have arrived), so only convert + store sit between "P V(i - 1)
+        // complete" and "V(i) ready".  (One warp per operand, not half a tile each: every mbarrier wait,
+        // fence and arrive costs a warp 120-200 clocks, measured with a clock trace.)
+        const int kv = warp - (2 + C::N_SOFTMAX / 32);
+        const uint32_t oper_full = bar(C::B_OPER + (kv ? O_VFULL : O_KFULL));
+        const uint32_t oper_empty = bar(C::B_OPER + (kv ? O_VEMPTY : O_KEMPTY));
+        uint8_t *dst = smem + C::OPER_OFF + kv * SLOT_BYTES;
         uint32_t ct = 0;                                  // tiles of all items so far
         for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = load_item(P.items, idx, P.seq_len);
@@ -307,37 +314,42 @@ attn_umma_kernel(const UParams P) {
             for (int i = 0; i < n_tiles; ++i, ++ct) {
                 const int nv = min(TILE_TOKENS, n_tok - i * TILE_TOKENS);
                 const int np = (nv + PS - 1) / PS;
+                const uint32_t ld = 2 * ct + kv, slot = ld % NSLOT, ph = (ld / NSLOT) & 1;
+                mbar_wait(bar(C::B_FULL + slot), ph);
+                const uint8_t *src = smem + C::RING_OFF + slot * C::RING_SLOT;
+                uint4 v[TILE_PAGES][4];
 #pragma unroll
-                for (int kv = 0; kv < 2; ++kv) {
-                    const uint32_t ld = 2 * ct + kv, slot = ld % NSLOT, ph = (ld / NSLOT) & 1;
-                    mbar_wait(bar(C::B_FULL + slot), ph);
-                    mbar_wait(bar(C::B_OPER + (kv ? O_VEMPTY : O_KEMPTY)), (ct & 1) ^ 1);
-                    const uint8_t *src = smem + C::RING_OFF + slot * C::RING_SLOT;
-                    uint8_t *dst = smem + C::OPER_OFF + kv * SLOT_BYTES;
-                    for (int pg = cw; pg < np; pg += 2) {
-                        const int valid = (kv && pg == np - 1 && (nv & (PS - 1))) ? (nv & (PS - 1)) : PS;
+                for (int pg = 0; pg < TILE_PAGES; ++pg)
 #pragma unroll
-                        for (int q4 = 0; q4 < 4; ++q4) {
-                            const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
-                            uint4 v = *reinterpret_cast<const uint4 *>(src + pg * (HEAD_BLOCK / 2) + row * 128 +
-                                                                       ((c8 ^ (row & 7)) << 4));
-                            uint4 a, b;
-                            e4m3x4_to_f16x4(v.x, a.x, a.y);
-                            e4m3x4_to_f16x4(v.y, a.z, a.w);
-                            e4m3x4_to_f16x4(v.z, b.x, b.y);
-                            e4m3x4_to_f16x4(v.w, b.z, b.w);
-                            if (row >= valid) a = b = make_uint4(0, 0, 0, 0);
-                            *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8)) = a;
-                            *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8 + 1)) = b;
-                        }
+                    for (int q4 = 0; q4 < 4; ++q4) {
+                        const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
+                        v[pg][q4] = pg < np ? *reinterpret_cast<const uint4 *>(src + pg * (HEAD_BLOCK / 2) + row * 128 +
+                                                                               ((c8 ^ (row & 7)) << 4))
+                                            : make_uint4(0, 0, 0, 0);
                     }
-                    fence_async_smem();
-                    __syncwarp();
-                    if (lane == 0) {
-                        mbar_arrive(bar(C::B_OPER + (kv ? O_VFULL : O_KFULL)));
-                        mbar_arrive(bar(C::B_EMPTY + slot));
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar(C::B_EMPTY + slot));      // the landing slot is free again
+                mbar_wait(oper_empty, (ct & 1) ^ 1);
+#pragma unroll
+                for (int pg = 0; pg < TILE_PAGES; ++pg) {
+                    if (pg >= np) continue;
+                    const int valid = (kv && pg == np - 1 && (nv & (PS - 1))) ? (nv & (PS - 1)) : PS;
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) {
+                        const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
+                        uint4 a, b;
+                        e4m3x4_to_f16x4(v[pg][q4].x, a.x, a.y);
+                        e4m3x4_to_f16x4(v[pg][q4].y, a.z, a.w);
+                        e4m3x4_to_f16x4(v[pg][q4].z, b.x, b.y);
+                        e4m3x4_to_f16x4(v[pg][q4].w, b.z, b.w);
+                        if (row >= valid) a = b = make_uint4(0, 0, 0, 0);
+                        *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8)) = a;
+                        *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8 + 1)) = b;
                     }
                 }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(oper_full);
             }
         }
     } else {
