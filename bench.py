@@ -428,8 +428,8 @@ def measure_attn(env: Env, spk, ids, cfg, wl, cpu=True):
                  "peak_source": peaks["_source"], "frac_of_8TBps": ach_bw / 8000.0,
                  "read_peak": read_peak, "frac_of_read_peak": ach_bw / read_peak,
                  "peak_note": "peak = MEASURED_PEAKS.json's copy (read + write) figure; read_peak = a plain "
-                              "read-only stream timed in this run (spork_hbm_read_probe), which a read-dominated "
-                              "kernel can exceed the copy figure up to",
+                              "read-only stream of bulk copies timed in this run (spork_hbm_read_probe), the "
+                              "ceiling of a read-dominated kernel",
                  "achieved_tflops": ach_tf, "algorithmic_bytes": ub, "algorithmic_flops": flops})
     warm = env.timed(st, step, args.steps, do_flush=False)
 

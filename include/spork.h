@@ -373,8 +373,9 @@ int spork_turn_sync(spork_turn *t, void *stream);
 int spork_turn_destroy(spork_turn *t);
 
 /*
- * Bench support: one read-only pass over `bytes` bytes at `buf` (device, 16-byte aligned), launched on
- * `stream`; the caller times it with events.  bench.py reports the rate it reaches (`read_peak`) beside
+ * Bench support: one read-only pass over `bytes` bytes at `buf` (device, 16-byte aligned; whole 16 KiB
+ * chunks are read), streamed like the attention kernel streams K/V (bulk copies into shared memory from
+ * 2 persistent CTAs per SM), launched on `stream`; the caller times it with events.  bench.py reports the rate it reaches (`read_peak`) beside
  * MEASURED_PEAKS.json's copy figure: the attention kernels are read streams (SURVEY.md 8(d) asks for GB/s
  * against the box's measured bandwidth).  Errors: SPORK_ERR_INVALID.
  */

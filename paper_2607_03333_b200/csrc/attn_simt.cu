@@ -215,6 +215,26 @@ __global__ void __launch_bounds__(128) merge_heads_kernel(const QRowDesc *__rest
         merge_row<NI>(rs, j, D, ws_o, ws_lse, out + (row0 + j) * D, lse + row0 + j, lane);
 }
 
+// one warp per (q row, kv head, group of 4 GQA heads): merge_heads4 (G % 4 == 0)
+template <int NI>
+__global__ void __launch_bounds__(128) merge_heads4_kernel(const QRowDesc *__restrict__ qd,
+                                                           const RowRef *__restrict__ refs,
+                                                           const StreamDesc *__restrict__ streams, int n_qrows,
+                                                           int Hq, int G, int D, const float *ws_o,
+                                                           const float *ws_lse, float *__restrict__ out,
+                                                           float *__restrict__ lse) {
+    const int Hkv = Hq / G, Q4 = G >> 2;
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n_qrows * Hkv * Q4) return;
+    const int qrow = w / (Hkv * Q4), kvh = (w / Q4) % Hkv, j0 = (w % Q4) * 4;
+    const QRowDesc d = qd[qrow];                 // written before the attention kernel was launched
+    const RowSplits rs = load_row_splits(d, refs, streams, kvh, lane);
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const size_t row0 = (size_t)qrow * Hq + (size_t)kvh * G + j0;
+    merge_heads4<NI>(rs, j0, D, ws_o, ws_lse, out + row0 * D, lse + row0, lane);
+}
+
 }  // namespace
 
 namespace spork {
@@ -257,7 +277,9 @@ int launch_merge(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
     // enough (q row, kv head) pairs to fill the SMs: the grouped kernel (measured: verify k = 16 merge
     // 60 -> 37 us, config 3 14 -> 12 us; config 2 / 5 with 256 / 512 pairs are faster per head)
     const bool grouped = P.n_qrows * c->cfg.num_kv_heads >= 1024;
-    const int warps = P.n_qrows * (grouped ? c->cfg.num_kv_heads : c->cfg.num_q_heads);
+    const bool by4 = grouped && c->G % 4 == 0 && c->cfg.head_dim <= 128;    // four heads per warp, four splits in flight
+    const int warps = P.n_qrows * (by4 ? c->cfg.num_kv_heads * (c->G / 4)
+                                       : (grouped ? c->cfg.num_kv_heads : c->cfg.num_q_heads));
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(ceil_div(warps, 4));
     cfg.blockDim = dim3(128);
@@ -267,8 +289,9 @@ int launch_merge(spork_ctx *c, const LayerIO &io, cudaStream_t st) {
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    auto kern = grouped ? (c->cfg.head_dim <= 128 ? merge_heads_kernel<1> : merge_heads_kernel<2>)
-                        : (c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>);
+    auto kern = by4 ? merge_heads4_kernel<1>
+                    : (grouped ? (c->cfg.head_dim <= 128 ? merge_heads_kernel<1> : merge_heads_kernel<2>)
+                               : (c->cfg.head_dim <= 128 ? merge_kernel<1> : merge_kernel<2>));
     SPORK_CUDA(cudaLaunchKernelEx(&cfg, kern, P.d_qdesc, P.d_refs, P.d_streams, P.n_qrows,
                                   (int)c->cfg.num_q_heads, c->G, (int)c->cfg.head_dim,
                                   (const float *)c->ws_o.p, (const float *)c->ws_lse.p,

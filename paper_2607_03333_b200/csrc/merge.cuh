@@ -196,4 +196,82 @@ __device__ __forceinline__ void merge_heads(const RowSplits &rs, int j0, int D, 
     }
 }
 
+// Four consecutive GQA heads of one (q row, kv head), FOUR splits in flight: every partial row of a batch
+// (4 splits x 4 heads x 512 B) and its lse are requested before anything is used, so a warp pays one memory
+// round trip per four splits instead of one per split plus one for the maxima (the merge is pure latency:
+// ncu showed 37 % long-scoreboard stalls at 20 warps per SM).  Batches are combined with a running maximum.
+// Lane e < 16 owns the weight of (split e / 4, head e % 4).
+template <int NI>
+__device__ __forceinline__ void merge_heads4(const RowSplits &rs, int j0, int D, const float *ws_o, const float *ws_lse,
+                                             float *out_rows, float *lse_out, int lane) {
+    const int n = rs.total, nv = D >> 2;
+    const int jj = lane & 3, sl = lane >> 2;
+    float4 acc[4][NI];
+    float W[4], M = -INFINITY;               // M: running maximum of head jj (the same on every lane with that jj)
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        W[k] = 0.f;
+#pragma unroll
+        for (int i = 0; i < NI; ++i) acc[k][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    for (int s0 = 0; s0 < n; s0 += 4) {
+        const int row_l = split_row(rs, s0 + sl, j0);                 // head j0's partial row of split s0 + sl
+        const bool mine = sl < 4 && row_l >= 0;
+        const float lse_l = mine ? __ldcg(ws_lse + row_l + jj) : -INFINITY;
+        float4 v[4][4][NI];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int row = __shfl_sync(0xffffffffu, row_l, u * 4);
+            const float4 *po = reinterpret_cast<const float4 *>(ws_o + (size_t)max(row, 0) * D);
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int c = lane + 32 * i;
+                    v[u][k][i] = (row >= 0 && c < nv) ? __ldcg(po + (size_t)k * nv + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+        }
+        float m = lse_l;
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, o));
+        const float M_new = fmaxf(M, m);
+        const float alpha_l = (M == -INFINITY) ? 0.f : expf(M - M_new);     // M_new = -inf: nothing yet, acc = 0 anyway
+        const float w_l = (mine && M_new != -INFINITY) ? expf(lse_l - M_new) : 0.f;
+        M = M_new;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const float alpha = __shfl_sync(0xffffffffu, alpha_l, k);
+            W[k] *= alpha;
+#pragma unroll
+            for (int i = 0; i < NI; ++i) {
+                acc[k][i].x *= alpha; acc[k][i].y *= alpha; acc[k][i].z *= alpha; acc[k][i].w *= alpha;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float w = __shfl_sync(0xffffffffu, w_l, u * 4 + k);
+                W[k] += w;
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    acc[k][i].x = fmaf(w, v[u][k][i].x, acc[k][i].x);
+                    acc[k][i].y = fmaf(w, v[u][k][i].y, acc[k][i].y);
+                    acc[k][i].z = fmaf(w, v[u][k][i].z, acc[k][i].z);
+                    acc[k][i].w = fmaf(w, v[u][k][i].w, acc[k][i].w);
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float inv = W[k] > 0.f ? 1.f / W[k] : 0.f;     // no partial / all empty: out = 0
+        float4 *o = reinterpret_cast<float4 *>(out_rows + (size_t)k * D);
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            const int c = lane + 32 * i;
+            if (c < nv) o[c] = make_float4(acc[k][i].x * inv, acc[k][i].y * inv, acc[k][i].z * inv, acc[k][i].w * inv);
+        }
+        const float Mk = __shfl_sync(0xffffffffu, M, k);     // lane k holds head k's maximum
+        if (lane == 0) lse_out[k] = W[k] > 0.f ? Mk + logf(W[k]) : -INFINITY;
+    }
+}
+
 }  // namespace spork
