@@ -59,10 +59,12 @@ __host__ __device__ constexpr bool emulated_pair(int j) { return (j * EMU_NUM) %
 //           4 per SM sub-partition instead of 2) for items whose time is the softmax's, not HBM's:
 //           4-slot ring, the row max and the row sums are exchanged through shared memory
 //   F8 (NP = SP = 1): the FP8-KV variant (e4m3 K/V bytes, bf16 Q).  The bulk copies land 8 KiB e4m3 tiles
-//           in a 6-slot ring; two converter warps (one for K, one for V) widen them (exactly) to fp16 into ONE
-//           K operand slot and ONE V operand slot in the same swizzled image the bf16 path stages directly, Q is converted
-//           bf16 -> fp16 when it is staged, P is packed as fp16: the MMAs run in kind::f16 with fp16
-//           operands, everything downstream of the operands is the bf16 kernel.
+//           in a 6-slot ring.  K is consumed where it lands: S = Q K^T runs in kind::f8f6f4, with Q split
+//           into TWO e4m3 terms when it is staged (q = hi + lo exactly for a bf16 q: 4 + 4 significant bits),
+//           so the scores are as exact as the bf16 path's.  V is widened (exactly) to fp16 by two converter
+//           warps, half a tile each, into one of TWO operand slots in the swizzled image the bf16 path
+//           stages directly; P is packed as fp16 and P V runs in kind::f16.  Softmax, epilogue, merge and
+//           planner are the bf16 kernel's.
 template <int NP, int SP, bool F8 = false>
 struct Cfg {
     static_assert(SP == 1 || NP == 1, "split rows only with one pipe");
@@ -74,7 +76,7 @@ struct Cfg {
     static constexpr int N_THREADS = 64 + N_SOFTMAX + N_CONV;
     static constexpr int CTAS_PER_SM = NP == 1 ? 2 : 1;
     static constexpr int TMEM_COLS = NP * PIPE_COLS;
-    static constexpr int OPER_OFF = NP * Q_BYTES;                         // F8: fp16 K slot, then fp16 V slot
+    static constexpr int OPER_OFF = NP * Q_BYTES;                         // F8: two fp16 V operand slots
     static constexpr int RING_OFF = OPER_OFF + (F8 ? 2 * SLOT_BYTES : 0);
     static constexpr int BAR_OFF = RING_OFF + NSLOT * RING_SLOT;
     // barrier slots (8 bytes each) from BAR_OFF
@@ -82,12 +84,13 @@ struct Cfg {
     static constexpr int B_EMPTY = NSLOT;             // [NSLOT] MMAs (F8: converters) reading the slot completed
     static constexpr int B_PIPE = 2 * NSLOT;          // per pipe: 7 barriers, see P_*
     static constexpr int B_QFULL = B_PIPE + 7 * NP;   // Q staged
-    static constexpr int B_OPER = B_QFULL + 1;        // F8: K slot full / empty, V slot full / empty
+    static constexpr int B_OPER = B_QFULL + 1;        // F8: V operand slot b full [2], empty [2]
     static constexpr int B_COUNT = B_OPER + (F8 ? 4 : 0);
     static constexpr int XCH_OFF = BAR_OFF + 8 * B_COUNT + 16;     // float [2][2][128] (SP = 2)
-    static constexpr int SMEM_BYTES = XCH_OFF + (SP == 2 ? 2048 : 0);
+    static constexpr int QEXP_OFF = XCH_OFF + (SP == 2 ? 2048 : 0);   // F8: uint8 [2][128], per-row power-of-two Q scaling
+    static constexpr int SMEM_BYTES = QEXP_OFF + (F8 ? 256 : 0);
 };
-enum : int { O_KFULL = 0, O_KEMPTY = 1, O_VFULL = 2, O_VEMPTY = 3 };
+enum : int { O_VFULL = 0, O_VEMPTY = 2 };
 enum : int {
     P_SFULL = 0,    // [2] S(b) complete
     P_PFULL = 2,    // [2] P(b) written (4 softmax warps)
@@ -128,7 +131,8 @@ attn_umma_kernel(const UParams P) {
         if (sbase & 1023u) __trap();   // the 128-byte swizzle is a function of the smem address
         for (int s = 0; s < NSLOT; ++s) {
             mbar_init(bar(C::B_FULL + s), 1);
-            mbar_init(bar(C::B_EMPTY + s), 1);
+            // F8: even slots hold K tiles (freed by the S MMAs' commit), odd slots V tiles (freed by both converter warps)
+            mbar_init(bar(C::B_EMPTY + s), (F8 && (s & 1)) ? 2 : 1);
         }
         for (int w = 0; w < NP; ++w) {
             for (int b = 0; b < 2; ++b) {
@@ -140,10 +144,10 @@ attn_umma_kernel(const UParams P) {
         }
         mbar_init(bar(C::B_QFULL), 1);
         if constexpr (F8) {
-            mbar_init(bar(C::B_OPER + O_KFULL), 1);     // the K converter warp
-            mbar_init(bar(C::B_OPER + O_VFULL), 1);     // the V converter warp
-            mbar_init(bar(C::B_OPER + O_KEMPTY), 1);    // tcgen05.commit
-            mbar_init(bar(C::B_OPER + O_VEMPTY), 1);
+            for (int b = 0; b < 2; ++b) {
+                mbar_init(bar(C::B_OPER + O_VFULL + b), 2);     // one arrival per converter warp
+                mbar_init(bar(C::B_OPER + O_VEMPTY + b), 1);    // tcgen05.commit
+            }
         }
         mbar_fence_init();
     }
@@ -209,8 +213,9 @@ attn_umma_kernel(const UParams P) {
         // one elected lane issues the tcgen05 instructions of a step.
         const uint64_t q_desc = smem_desc_sw128(sbase, 16, 1024);     // K-major, 8-row groups 1 KiB apart
         // operand tiles: the ring itself, or (F8) the two fp16 slots the converter warps fill
-        const uint32_t k_base = F8 ? sbase + C::OPER_OFF : ring, v_base = F8 ? sbase + C::OPER_OFF + SLOT_BYTES : ring;
-        const uint64_t k_desc = smem_desc_sw128(k_base, 16, 2048);      // K-major, 8-token groups 2 KiB apart
+        const uint32_t v_base = F8 ? sbase + C::OPER_OFF : ring;
+        // K-major, 8-token groups 2 KiB apart (e4m3: 128-byte rows hold all 128 dims, groups 1 KiB apart)
+        const uint64_t k_desc = smem_desc_sw128(ring, 16, F8 ? 1024 : 2048);
         const uint64_t v_desc = smem_desc_sw128(v_base, 1024, 2048);    // MN-major: dim halves 1 KiB, 8-token groups 2 KiB
         constexpr uint32_t ID_PV = F8 ? idesc_f16(128, D, 0, 1) : idesc_bf16(128, D, 0, 1);
         uint32_t gt = 0;            // tiles of all items so far: K of tile gt is load 2 gt, V is 2 gt + 1
@@ -229,27 +234,33 @@ attn_umma_kernel(const UParams P) {
             };
             auto issue_s = [&](int i) {
                 const uint32_t ldk = 2 * (gt + i);
-                const uint32_t slot = F8 ? 0 : ldk % NSLOT, ph = F8 ? (gt + i) & 1 : (ldk / NSLOT) & 1;
-                const uint32_t k_full = F8 ? bar(C::B_OPER + O_KFULL) : bar(C::B_FULL + slot);
-                const uint32_t k_empty = F8 ? bar(C::B_OPER + O_KEMPTY) : bar(C::B_EMPTY + slot);
-                mbar_wait(k_full, ph);
+                const uint32_t slot = ldk % NSLOT, ph = (ldk / NSLOT) & 1;
+                mbar_wait(bar(C::B_FULL + slot), ph);
                 tc_fence_after();
                 const uint32_t id = F8 ? idesc_f16(128, PS * pages_of_tile(i), 0, 0) : idesc_bf16(128, PS * pages_of_tile(i), 0, 0);
-                const uint64_t kd = smem_desc_advance(k_desc, slot * SLOT_BYTES);
+                const uint64_t kd = smem_desc_advance(k_desc, slot * C::RING_SLOT);
                 if (elect_one()) {
 #pragma unroll
                     for (int w = 0; w < NP; ++w) {
                         if (w < npipe) {
                             const uint32_t b = (g0[w] + i) & 1;
                             const uint32_t tS = tbase + w * PIPE_COLS + 128 + 64 * b;
+                            if constexpr (F8) {
+                                // 4 K-steps of 32 e4m3 dims, for the hi and the lo term of Q (16 KiB apart)
 #pragma unroll
-                            for (int ks = 0; ks < 8; ++ks)
-                                mma_ss(tS, smem_desc_advance(q_desc, w * Q_BYTES + (ks >> 2) * Q_HALF + (ks & 3) * 32),
-                                       smem_desc_advance(kd, (ks >> 2) * 1024 + (ks & 3) * 32), id, ks > 0);
+                                for (int ks = 0; ks < 8; ++ks)
+                                    mma_ss_f8(tS, smem_desc_advance(q_desc, (ks >> 2) * Q_HALF + (ks & 3) * 32),
+                                              smem_desc_advance(kd, (ks & 3) * 32), id, ks > 0);
+                            } else {
+#pragma unroll
+                                for (int ks = 0; ks < 8; ++ks)
+                                    mma_ss(tS, smem_desc_advance(q_desc, w * Q_BYTES + (ks >> 2) * Q_HALF + (ks & 3) * 32),
+                                           smem_desc_advance(kd, (ks >> 2) * 1024 + (ks & 3) * 32), id, ks > 0);
+                            }
                             mma_commit(pbar(w, P_SFULL + b));
                         }
                     }
-                    mma_commit(k_empty);
+                    mma_commit(bar(C::B_EMPTY + slot));
                 }
                 __syncwarp();
             };
@@ -259,9 +270,10 @@ attn_umma_kernel(const UParams P) {
             for (int i = 0; i < n_tiles; ++i) {
                 if (i + 1 < n_tiles) issue_s(i + 1);
                 const uint32_t ldv = 2 * (gt + i) + 1;
-                const uint32_t slot = F8 ? 0 : ldv % NSLOT, ph = F8 ? (gt + i) & 1 : (ldv / NSLOT) & 1;
-                const uint32_t v_full = F8 ? bar(C::B_OPER + O_VFULL) : bar(C::B_FULL + slot);
-                const uint32_t v_empty = F8 ? bar(C::B_OPER + O_VEMPTY) : bar(C::B_EMPTY + slot);
+                // F8: tile T's V sits in operand slot T & 1, filled by the converter warps
+                const uint32_t slot = F8 ? (gt + i) & 1 : ldv % NSLOT, ph = F8 ? ((gt + i) >> 1) & 1 : (ldv / NSLOT) & 1;
+                const uint32_t v_full = F8 ? bar(C::B_OPER + O_VFULL + slot) : bar(C::B_FULL + slot);
+                const uint32_t v_empty = F8 ? bar(C::B_OPER + O_VEMPTY + slot) : bar(C::B_EMPTY + slot);
                 const uint64_t vd = smem_desc_advance(v_desc, slot * SLOT_BYTES);
                 const int nvp = pages_of_tile(i);
 #pragma unroll
@@ -293,19 +305,14 @@ attn_umma_kernel(const UParams P) {
         }
     } else if (F8 && warp >= 2 + C::N_SOFTMAX / 32) {
         // ================================ converter warps (FP8-KV) ================================
-        // Warp 0 of the two widens every landed K tile, warp 1 every V tile, e4m3 -> fp16 (exact), into the K
-        // / V operand slot: the same block image the bf16 path stages directly (swz_chunk_off(2, ...)).
-        // The e4m3 block is 16 rows of 128 bytes, 16-byte chunks XOR-swizzled by (row & 7); a quarter warp
-        // takes one chunk column of 8 rows, which is conflict-free for the loads and for the stores.
-        // Rows of a partially filled last V page are written as zeros (pool memory may hold NaN codes).
-        // A tile's 16 loads are issued before the warp waits for its operand slot (the landing slot is
-        // released as soon as they have arrived), so only convert + store sit between "P V(i - 1)
-        // complete" and "V(i) ready".  (One warp per operand, not half a tile each: every mbarrier wait,
-        // fence and arrive costs a warp 120-200 clocks, measured with a clock trace.)
-        const int kv = warp - (2 + C::N_SOFTMAX / 32);
-        const uint32_t oper_full = bar(C::B_OPER + (kv ? O_VFULL : O_KFULL));
-        const uint32_t oper_empty = bar(C::B_OPER + (kv ? O_VEMPTY : O_KEMPTY));
-        uint8_t *dst = smem + C::OPER_OFF + kv * SLOT_BYTES;
+        // Warp cw widens pages cw and cw + 2 of every landed V tile, e4m3 -> fp16 (exact), into V operand
+        // slot (tile & 1): the block image the bf16 path stages directly (swz_chunk_off(2, ...)).  The e4m3
+        // block is 16 rows of 128 bytes, 16-byte chunks XOR-swizzled by (row & 7); a quarter warp takes one
+        // chunk column of 8 rows, which is conflict-free for the loads and for the stores.  Rows of a
+        // partially filled last page are written as zeros (pool memory may hold NaN codes).  A tile's
+        // loads are issued before the warp waits for its operand slot and the landing slot is released as
+        // soon as they have arrived.  (K is not widened: the S MMAs read the landed e4m3 tile.)
+        const int cw = warp - (2 + C::N_SOFTMAX / 32);
         uint32_t ct = 0;                                  // tiles of all items so far
         for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = load_item(P.items, idx, P.seq_len);
@@ -314,34 +321,36 @@ attn_umma_kernel(const UParams P) {
             for (int i = 0; i < n_tiles; ++i, ++ct) {
                 const int nv = min(TILE_TOKENS, n_tok - i * TILE_TOKENS);
                 const int np = (nv + PS - 1) / PS;
-                const uint32_t ld = 2 * ct + kv, slot = ld % NSLOT, ph = (ld / NSLOT) & 1;
+                const uint32_t ld = 2 * ct + 1, slot = ld % NSLOT, ph = (ld / NSLOT) & 1, vb = ct & 1;
                 mbar_wait(bar(C::B_FULL + slot), ph);
                 const uint8_t *src = smem + C::RING_OFF + slot * C::RING_SLOT;
-                uint4 v[TILE_PAGES][4];
+                uint8_t *dst = smem + C::OPER_OFF + vb * SLOT_BYTES;
+                uint4 v[2][4];
 #pragma unroll
-                for (int pg = 0; pg < TILE_PAGES; ++pg)
+                for (int u = 0; u < 2; ++u)
 #pragma unroll
                     for (int q4 = 0; q4 < 4; ++q4) {
-                        const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
-                        v[pg][q4] = pg < np ? *reinterpret_cast<const uint4 *>(src + pg * (HEAD_BLOCK / 2) + row * 128 +
-                                                                               ((c8 ^ (row & 7)) << 4))
-                                            : make_uint4(0, 0, 0, 0);
+                        const int pg = cw + 2 * u, row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
+                        v[u][q4] = pg < np ? *reinterpret_cast<const uint4 *>(src + pg * (HEAD_BLOCK / 2) + row * 128 +
+                                                                              ((c8 ^ (row & 7)) << 4))
+                                           : make_uint4(0, 0, 0, 0);
                     }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar(C::B_EMPTY + slot));      // the landing slot is free again
-                mbar_wait(oper_empty, (ct & 1) ^ 1);
+                mbar_wait(bar(C::B_OPER + O_VEMPTY + vb), ((ct >> 1) & 1) ^ 1);
 #pragma unroll
-                for (int pg = 0; pg < TILE_PAGES; ++pg) {
+                for (int u = 0; u < 2; ++u) {
+                    const int pg = cw + 2 * u;
                     if (pg >= np) continue;
-                    const int valid = (kv && pg == np - 1 && (nv & (PS - 1))) ? (nv & (PS - 1)) : PS;
+                    const int valid = (pg == np - 1 && (nv & (PS - 1))) ? (nv & (PS - 1)) : PS;
 #pragma unroll
                     for (int q4 = 0; q4 < 4; ++q4) {
                         const int row = (lane & 7) + 8 * (q4 & 1), c8 = (lane >> 3) + 4 * (q4 >> 1);
                         uint4 a, b;
-                        e4m3x4_to_f16x4(v[pg][q4].x, a.x, a.y);
-                        e4m3x4_to_f16x4(v[pg][q4].y, a.z, a.w);
-                        e4m3x4_to_f16x4(v[pg][q4].z, b.x, b.y);
-                        e4m3x4_to_f16x4(v[pg][q4].w, b.z, b.w);
+                        e4m3x4_to_f16x4(v[u][q4].x, a.x, a.y);
+                        e4m3x4_to_f16x4(v[u][q4].y, a.z, a.w);
+                        e4m3x4_to_f16x4(v[u][q4].z, b.x, b.y);
+                        e4m3x4_to_f16x4(v[u][q4].w, b.z, b.w);
                         if (row >= valid) a = b = make_uint4(0, 0, 0, 0);
                         *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8)) = a;
                         *reinterpret_cast<uint4 *>(dst + pg * HEAD_BLOCK + swz_chunk_off(2, row, 2 * c8 + 1)) = b;
@@ -349,7 +358,7 @@ attn_umma_kernel(const UParams P) {
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(oper_full);
+                if (lane == 0) mbar_arrive(bar(C::B_OPER + O_VFULL + vb));
             }
         }
     } else {
@@ -367,7 +376,7 @@ attn_umma_kernel(const UParams P) {
         // NEXT item as soon as this thread has seen the last S of the current item complete (its Q
         // image is then dead), i.e. before the epilogue: the global-load latency and the next item's
         // first S MMA hide under the last P V and the write-back of the partials.
-        auto stage_q = [&](const WorkItem &qi) {
+        auto stage_q = [&](const WorkItem &qi, int parity) {
             const int c = st & 15;                     // 16-byte chunk of the row
             constexpr int QT = 128 * SP, NK = 16 / SP;  // threads staging one pipe's image, rows per thread
             uint4 v[NK];
@@ -375,25 +384,62 @@ attn_umma_kernel(const UParams P) {
             for (int k = 0; k < NK; ++k) {
                 const int row = w * 128 + ((st & (QT - 1)) >> 4) + (QT / 16) * k;
                 v[k] = make_uint4(0, 0, 0, 0);
+                if (F8 && c == 0 && row >= qi.nrows) smem[C::QEXP_OFF + parity * 128 + (row & 127)] = 134;   // scale 1
                 if (row < qi.nrows) {
                     const int lr = qi.rb0 + row;
                     const uint16_t *src =
                         P.q + ((size_t)item_qrow(qi, P.rowmap, lr, P.G) * P.Hq + qi.kvh * P.G + lr % P.G) * D + c * 8;
                     v[k] = *reinterpret_cast<const uint4 *>(src);
-                    if constexpr (F8) {       // bf16 -> fp16 (exact within fp16's range; beyond it saturates)
-                        uint32_t *u = reinterpret_cast<uint32_t *>(&v[k]);
+                    if constexpr (F8) {
+                        // bf16 -> two e4m3 terms, q * 2^s = hi + lo: the row is first scaled by the power of two
+                        // that brings its largest magnitude into [128, 256) (e4m3 tops out at 448; the softmax
+                        // thread of the row undoes it in its score scale), hi = the scaled q rounded to e4m3
+                        // (4 significant bits), lo = the residual, again e4m3: exact for a bf16 q (8 significant
+                        // bits) down to elements 2^-17 of the row's largest.  The 8 hi bytes go to v[k].x/.y,
+                        // the 8 lo bytes to v[k].z/.w.
+                        const uint32_t *u = reinterpret_cast<const uint32_t *>(&v[k]);
+                        float mx = 0.f;
 #pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            const float lo = fminf(fmaxf(__uint_as_float(u[e] << 16), -65504.f), 65504.f);
-                            const float hi = fminf(fmaxf(__uint_as_float(u[e] & 0xffff0000u), -65504.f), 65504.f);
-                            u[e] = pack_f16(lo, hi);
+                        for (int e = 0; e < 4; ++e)
+                            mx = fmaxf(mx, fmaxf(fabsf(__uint_as_float(u[e] << 16)), fabsf(__uint_as_float(u[e] & 0xffff0000u))));
+#pragma unroll
+                        for (int o = 1; o < 16; o <<= 1)       // the row's 16 chunks = one half warp (the other half may sit this row out)
+                            mx = fmaxf(mx, __shfl_xor_sync(lane < 16 ? 0x0000ffffu : 0xffff0000u, mx, o));
+                        uint32_t eb = (__float_as_uint(mx) >> 23) & 0xffu;       // biased exponent of the row maximum
+                        eb = min(max(eb, 32u), 220u);                            // (zero / tiny / huge rows: a harmless scale)
+                        const float qs = __uint_as_float((261u - eb) << 23);    // 2^(7 - e)
+                        if (c == 0) smem[C::QEXP_OFF + parity * 128 + row] = (uint8_t)eb;
+                        uint32_t hi8[2], lo8[2];
+#pragma unroll
+                        for (int e2 = 0; e2 < 2; ++e2) {
+                            float f[4], g[4];
+                            f[0] = __uint_as_float(u[2 * e2] << 16) * qs;
+                            f[1] = __uint_as_float(u[2 * e2] & 0xffff0000u) * qs;
+                            f[2] = __uint_as_float(u[2 * e2 + 1] << 16) * qs;
+                            f[3] = __uint_as_float(u[2 * e2 + 1] & 0xffff0000u) * qs;
+                            const uint32_t h = pack_e4m3(f[0], f[1]) | (pack_e4m3(f[2], f[3]) << 16);
+                            uint32_t h01, h23;
+                            e4m3x4_to_f16x4(h, h01, h23);
+                            unpack_f16(h01, g[0], g[1]);
+                            unpack_f16(h23, g[2], g[3]);
+                            hi8[e2] = h;
+                            lo8[e2] = pack_e4m3(f[0] - g[0], f[1] - g[1]) | (pack_e4m3(f[2] - g[2], f[3] - g[3]) << 16);
                         }
+                        v[k] = make_uint4(hi8[0], hi8[1], lo8[0], lo8[1]);
                     }
                 }
             }
 #pragma unroll
             for (int k = 0; k < NK; ++k) {
                 const int rp = ((st & (QT - 1)) >> 4) + (QT / 16) * k;   // row inside the pipe's 32 KiB image
+                if constexpr (F8) {
+                    // e4m3 images: rows of 128 bytes (all 128 dims), 16-byte chunks XOR-swizzled by the row;
+                    // chunk c of the bf16 row (8 dims) is half of e4m3 chunk c / 2; hi image, lo image 16 KiB on
+                    const int off = (rp >> 3) * 1024 + (rp & 7) * 128 + ((((c >> 1) & 7) ^ (rp & 7)) << 4) + (c & 1) * 8;
+                    *reinterpret_cast<uint2 *>(smem + off) = make_uint2(v[k].x, v[k].y);
+                    *reinterpret_cast<uint2 *>(smem + Q_HALF + off) = make_uint2(v[k].z, v[k].w);
+                    continue;
+                }
                 const int off = w * Q_BYTES + (c >> 3) * Q_HALF + (rp >> 3) * 1024 + (rp & 7) * 128 +
                                 (((c & 7) ^ (rp & 7)) << 4);
                 *reinterpret_cast<uint4 *>(smem + off) = v[k];
@@ -402,7 +448,7 @@ attn_umma_kernel(const UParams P) {
             asm volatile("bar.sync 1, %0;" ::"n"(C::N_SOFTMAX) : "memory");
             if (st == 0) mbar_arrive(bar(C::B_QFULL));
         };
-        if (item_begin < item_end) stage_q(P.items[item_begin]);
+        if (item_begin < item_end) stage_q(P.items[item_begin], 0);
         for (int idx = item_begin; idx < item_end; ++idx) {
             const WorkItem it = load_item(P.items, idx, P.seq_len);
             const bool has_next = idx + 1 < item_end;
@@ -415,6 +461,12 @@ attn_umma_kernel(const UParams P) {
             const int lim_r = it.lim0 + (it.rb0 + r) / P.G;
             const int min_lim = it.lim0 + (it.rb0 + w * 128) / P.G;
             float m_used = -INFINITY, l = 0.f, lr = 0.f;   // l: exact row sum (lse); lr: sum of the bf16 weights
+            // score scale of this thread's row (log2 domain); F8: times the inverse of the row's Q scaling
+            float scale_log2 = P.scale_log2;
+            if constexpr (F8) {
+                const uint32_t eb = smem[C::QEXP_OFF + ((idx - item_begin) & 1) * 128 + (r & 127)];
+                scale_log2 *= __uint_as_float((eb - 7u) << 23);                  // 2^(e - 7)
+            }
 
             if (mode == 1) {
                 for (int i = 0; i < n_tiles; ++i) {
@@ -517,7 +569,7 @@ attn_umma_kernel(const UParams P) {
                     __syncwarp();
                     if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
                 }
-                if (has_next) stage_q(P.items[idx + 1]);
+                if (has_next) stage_q(P.items[idx + 1], (idx + 1 - item_begin) & 1);
                 if (mode == 1) {
                     const uint32_t gl = g0 + n_tiles - 1;
                     mbar_wait(pbar(w, P_PVDONE + (gl & 1)), (gl >> 1) & 1);
@@ -585,7 +637,7 @@ attn_umma_kernel(const UParams P) {
                 for (int t = 0; t < 32; ++t)
                     mxa[t & 3] = fmaxf(mxa[t & 3], fmaxf(__uint_as_float(s0[t]), __uint_as_float(s1[t])));
                 const float mx = fmaxf(fmaxf(mxa[0], mxa[1]), fmaxf(mxa[2], mxa[3]));
-                const float mxs = mx * P.scale_log2;
+                const float mxs = mx * scale_log2;
                 const bool grow = mxs > m_used + RESCALE_THRESHOLD;
                 if (__any_sync(0xffffffffu, grow)) {
                     const float m_new = grow ? mxs : m_used;
@@ -617,8 +669,8 @@ attn_umma_kernel(const UParams P) {
 #pragma unroll
                 for (int t = 0; t < 16; ++t) {
                     float x0, x1, y0, y1;
-                    ffma2(x0, x1, __uint_as_float(s0[2 * t]), __uint_as_float(s0[2 * t + 1]), P.scale_log2, nmu);
-                    ffma2(y0, y1, __uint_as_float(s1[2 * t]), __uint_as_float(s1[2 * t + 1]), P.scale_log2, nmu);
+                    ffma2(x0, x1, __uint_as_float(s0[2 * t]), __uint_as_float(s0[2 * t + 1]), scale_log2, nmu);
+                    ffma2(y0, y1, __uint_as_float(s1[2 * t]), __uint_as_float(s1[2 * t + 1]), scale_log2, nmu);
                     float a0, a1, c0, c1;
                     if (emulated_pair(2 * t)) ex2_poly2(x0, x1, a0, a1); else { a0 = ex2(x0); a1 = ex2(x1); }
                     if (emulated_pair(2 * t + 1)) ex2_poly2(y0, y1, c0, c1); else { c0 = ex2(y0); c1 = ex2(y1); }
@@ -666,7 +718,7 @@ attn_umma_kernel(const UParams P) {
                 if (lane == 0) mbar_arrive(pbar(w, P_PFULL + b));
             }
 
-            if (has_next) stage_q(P.items[idx + 1]);
+            if (has_next) stage_q(P.items[idx + 1], (idx + 1 - item_begin) & 1);
 
             if (mode == 1) {
                 const uint32_t gl = g0 + n_tiles - 1;
