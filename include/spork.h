@@ -68,8 +68,7 @@ typedef struct spork_ctx spork_ctx;
 
 typedef struct spork_config {
     int32_t dtype;             /* SPORK_F32 | SPORK_BF16: storage type of K, V and Q;
-                                  SPORK_E4M3: K and V are e4m3 bytes, Q is bf16 (queries
-                                  beyond fp16's range, |q| > 65504, saturate there)        */
+                                  SPORK_E4M3: K and V are e4m3 bytes, Q is bf16            */
     int32_t num_q_heads;       /* Hq                                                    */
     int32_t num_kv_heads;      /* Hkv, divides Hq; q head h reads kv head h/(Hq/Hkv)    */
     int32_t head_dim;          /* D: multiple of 32, <= 256                             */
