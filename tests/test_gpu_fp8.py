@@ -140,3 +140,29 @@ def test_full_config2_shape_in_e4m3_every_row():
     info = spk.last_plan()
     assert info["kernel"] == 2 and info["stream_k"] == 1 and info["unique_tokens"] == wl.unique_tokens()
     check_attn(out, lse, ref, lref, "e4m3", "cfg2 shape, e4m3 KV (all rows)")
+
+
+def test_full_config5_shape_in_e4m3_every_row():
+    """BASELINE.json config 5's batch (128 sequences, prefix 32768) with an e4m3 cache: the whole step against the
+    oracle, and the 36-layer-style chained call on two layers of it."""
+    import torch
+    cfg = f8(synth.CFG5)
+    wl, orc, spk, ids = _build_both(cfg)
+    assert_state_equal(orc, spk, ids)
+    q = wl.q_all()
+    ref, lref = orc.decode(ids, q)
+    out, lse = spk.decode_attn(wl.group_indptr(), ids, q)
+    info = spk.last_plan()
+    assert info["kernel"] == 2 and info["stream_k"] == 1 and info["unique_tokens"] == wl.unique_tokens()
+    check_attn(out, lse, ref, lref, "e4m3", "cfg5 shape, e4m3 KV (all rows)")
+    # two layers over the same tables (layer 1 = a copy of layer 0's pools): one plan, chained launches
+    spk.layers(2)
+    with torch.cuda.stream(spk.stream):
+        spk.k_pools[1].copy_(spk.k_pool)
+        spk.v_pools[1].copy_(spk.v_pool)
+    qd = spk._dev(q)
+    outs = [torch.empty_like(out) for _ in range(2)]
+    lses = [torch.empty_like(lse) for _ in range(2)]
+    spk.attn_layers(wl.group_indptr(), ids, [qd, qd], outs, lses)
+    for l in range(2):
+        check_attn(outs[l], lses[l], ref, lref, "e4m3", f"cfg5 e4m3, layer {l} of a chained call")

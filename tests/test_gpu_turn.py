@@ -21,6 +21,7 @@ def _inputs(cfg, ks, turn, accept_upto):
     r = synth.rng(cfg.cfg_no, synth.T_MISC, 1000 + turn)
     tot, n = int(ks.sum()), len(ks)
     f = lambda *shape: synth.to_storage(r.standard_normal(shape, dtype=np.float32), cfg.dtype)
+    fq = lambda *shape: synth.to_storage(r.standard_normal(shape, dtype=np.float32), cfg.q_dtype)
     draft = r.integers(0, 50000, size=tot).astype(np.int32)
     target = draft.copy()
     qi = np.concatenate([[0], np.cumsum(ks)])
@@ -29,14 +30,15 @@ def _inputs(cfg, ks, turn, accept_upto):
         if a < ks[i]:
             target[qi[i] + a] += 1
             target[qi[i] + a + 1:qi[i + 1]] = r.integers(0, 50000, size=int(ks[i]) - a - 1)
-    return dict(kd=f(tot, cfg.Hkv, cfg.D), vd=f(tot, cfg.Hkv, cfg.D), qv=f(tot, cfg.Hq, cfg.D), draft=draft,
-                target=target, k1=f(n, cfg.Hkv, cfg.D), v1=f(n, cfg.Hkv, cfg.D), qd=f(n, cfg.Hq, cfg.D))
+    return dict(kd=f(tot, cfg.Hkv, cfg.D), vd=f(tot, cfg.Hkv, cfg.D), qv=fq(tot, cfg.Hq, cfg.D), draft=draft,
+                target=target, k1=f(n, cfg.Hkv, cfg.D), v1=f(n, cfg.Hkv, cfg.D), qd=fq(n, cfg.Hq, cfg.D))
 
 
-@pytest.mark.parametrize("ks,n_turns", [([16, 16, 16, 16], 20), ([4, 9, 16, 1], 20), ([64, 33, 17, 2], 6)])
-def test_graph_replay_matches_the_oracle_turn_by_turn(ks, n_turns):
+@pytest.mark.parametrize("ks,n_turns,dtype", [([16, 16, 16, 16], 20, "bf16"), ([4, 9, 16, 1], 20, "bf16"),
+                                              ([64, 33, 17, 2], 6, "bf16"), ([8, 3, 16, 5], 8, "e4m3")])
+def test_graph_replay_matches_the_oracle_turn_by_turn(ks, n_turns, dtype):
     import torch
-    cfg = synth.CFG4.scaled(n_groups=2, prefix_len=1024 + 32, suffix_lo=0, suffix_hi=100, k_draft=0)
+    cfg = synth.CFG4.scaled(n_groups=2, prefix_len=1024 + 32, suffix_lo=0, suffix_hi=100, k_draft=0, dtype=dtype)
     wl = synth.Workload(cfg)
     ks = np.array(ks * cfg.n_groups, np.int64)
     grow = int(n_turns * (ks.max() + 1) + ks.max())
@@ -76,8 +78,8 @@ def test_graph_replay_matches_the_oracle_turn_by_turn(ks, n_turns):
         assert turn.sync() == 0
         (ov, lv), a, (od, ld) = oracle_turn(x)
         assert np.array_equal(acc.cpu().numpy(), a), what
-        check_attn(out_v, lse_v, ov, lv, "bf16", what + " verify")
-        check_attn(out_d, lse_d, od, ld, "bf16", what + " decode")
+        check_attn(out_v, lse_v, ov, lv, dtype, what + " verify")
+        check_attn(out_d, lse_d, od, ld, dtype, what + " decode")
         assert_state_equal(orc, spk, ids)
 
     # turn 0 eagerly (also the warm-up the capture needs), then the same calls captured once
