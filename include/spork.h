@@ -357,7 +357,9 @@ int spork_verify_attn_layers(spork_ctx *ctx, int n_layers, int n_groups, const i
  * From the first turn call on the host's copy of the lengths is stale: every other state or attention
  * call returns SPORK_ERR_STALE until spork_turn_sync (which synchronises `stream`, reads the lengths and
  * the free-page count back, and returns SPORK_ERR_DEVICE if a turn ran out of pages or block-table row --
- * such an append leaves the state untouched, as the host path does).  After a sync the graph can go on
+ * such an append leaves the state untouched, as the host path does -- or if spork_turn_accept was asked to
+ * roll a sequence back below its length at spork_turn_prepare, i.e. to reject drafts the turn did not
+ * append: that sequence is left alone).  After a sync the graph can go on
  * being replayed.  Errors: INVALID, INVALID_SEQ, STALE, CUDA.
  */
 typedef struct spork_turn spork_turn;

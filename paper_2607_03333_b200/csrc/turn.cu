@@ -33,10 +33,10 @@ struct spork_turn {
     Plan plan_v, plan_d;            // verify (k_i rows per sequence) and decode (one row) plans
     int need_ub[2] = {0, 0};        // upper bound on the pages an append of kind 0 (drafts) / 1 (one token) takes
     int total_tok[2] = {0, 0};
-    // one device buffer: seq_ids[n], n_tok[2][n], tok_off[2][n], q_indptr[n + 1], AppendDesc[n]
+    // one device buffer: seq_ids[n], n_tok[2][n], tok_off[2][n], base_len[n], q_indptr[n + 1], AppendDesc[n]
     DevBuf dev;
     const int32_t *d_seq = nullptr, *d_ntok[2] = {nullptr, nullptr}, *d_tokoff[2] = {nullptr, nullptr};
-    const int32_t *d_qi = nullptr;
+    const int32_t *d_qi = nullptr, *d_base = nullptr;
     AppendDesc *d_descs = nullptr;
 };
 
@@ -95,12 +95,14 @@ __global__ void __launch_bounds__(256) turn_append_plan_kernel(const int32_t *__
 
 // One warp per sequence: accept length = leading positions with draft == target, the
 // rejected drafts' pages are dropped and the length is rolled back, all from the device length.  The kept
-// tail page cannot be shared when the drafts are the tokens the turn appended; should it be, the sequence
-// is left alone and the sticky error word is set.
+// tail page cannot be shared, and the new length cannot fall below the length at spork_turn_prepare, when
+// the drafts are the tokens the turn appended; should either happen, the sequence is left alone and the
+// sticky error word is set.
 __global__ void __launch_bounds__(128) turn_accept_kernel(const int32_t *__restrict__ seq,
                                                           const int32_t *__restrict__ q_indptr,
                                                           const int32_t *__restrict__ draft,
-                                                          const int32_t *__restrict__ target, int n, int32_t *len,
+                                                          const int32_t *__restrict__ target,
+                                                          const int32_t *__restrict__ base_len, int n, int32_t *len,
                                                           int32_t *table, int table_stride, int32_t *refcount,
                                                           int32_t *counters, int32_t *__restrict__ accept_out) {
     const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -119,7 +121,8 @@ __global__ void __launch_bounds__(128) turn_accept_kernel(const int32_t *__restr
     const int s = seq[w], L = len[s], newL = L - (k - a);
     if (newL == L) return;
     int32_t *row = table + (size_t)s * table_stride;
-    if (newL < 0 || ((newL % PS) && refcount[row[newL / PS]] > 1)) {
+    // (below the length the plans were built for, their fixed pieces would reach past the sequence)
+    if (newL < base_len[w] || ((newL % PS) && refcount[row[newL / PS]] > 1)) {
         if (lane == 0) atomicExch(&counters[1], 4);
         return;
     }
@@ -193,7 +196,8 @@ extern "C" int spork_turn_prepare(spork_ctx *c, int n_groups, const int32_t *gro
     // ---- descriptors that stay put on the device ----
     const size_t o_seq = 0, o_nt0 = al16(o_seq + 4 * (size_t)n), o_nt1 = al16(o_nt0 + 4 * (size_t)n);
     const size_t o_to0 = al16(o_nt1 + 4 * (size_t)n), o_to1 = al16(o_to0 + 4 * (size_t)n);
-    const size_t o_qi = al16(o_to1 + 4 * (size_t)n), o_desc = al16(o_qi + 4 * (size_t)(n + 1));
+    const size_t o_base = al16(o_to1 + 4 * (size_t)n);
+    const size_t o_qi = al16(o_base + 4 * (size_t)n), o_desc = al16(o_qi + 4 * (size_t)(n + 1));
     const size_t total = o_desc + sizeof(AppendDesc) * (size_t)n;
     if (rc == SPORK_OK) rc = devbuf_reserve(&t->dev, total, st);
     if (rc == SPORK_OK && (size_t)t->need_ub[0] > c->free_list_cap) {      // grow now: no reallocation under capture
@@ -211,6 +215,7 @@ extern "C" int spork_turn_prepare(spork_ctx *c, int n_groups, const int32_t *gro
         int32_t *nt0 = (int32_t *)(h + o_nt0), *nt1 = (int32_t *)(h + o_nt1);
         int32_t *to0 = (int32_t *)(h + o_to0), *to1 = (int32_t *)(h + o_to1);
         memcpy(h + o_seq, seq_ids, 4 * (size_t)n);
+        memcpy(h + o_base, t->base_len.data(), 4 * (size_t)n);
         memcpy(h + o_qi, q_indptr, 4 * (size_t)(n + 1));
         for (int i = 0; i < n; ++i) {
             nt0[i] = t->k[i];
@@ -232,6 +237,7 @@ extern "C" int spork_turn_prepare(spork_ctx *c, int n_groups, const int32_t *gro
     t->d_tokoff[0] = (const int32_t *)(d + o_to0);
     t->d_tokoff[1] = (const int32_t *)(d + o_to1);
     t->d_qi = (const int32_t *)(d + o_qi);
+    t->d_base = (const int32_t *)(d + o_base);
     t->d_descs = (AppendDesc *)(d + o_desc);
     t->structure_epoch = c->structure_epoch;
     *out = t;
@@ -290,7 +296,7 @@ extern "C" int spork_turn_accept(spork_turn *t, const int32_t *draft_tokens, con
     c->mirror_stale = true;
     c->fl_valid = false;
     turn_accept_kernel<<<ceil_div(t->n_seq, 4), 128, 0, (cudaStream_t)stream>>>(
-        t->d_seq, t->d_qi, draft_tokens, target_tokens, t->n_seq, c->d_len, c->d_table, c->table_stride,
+        t->d_seq, t->d_qi, draft_tokens, target_tokens, t->d_base, t->n_seq, c->d_len, c->d_table, c->table_stride,
         c->d_refcount, c->d_counters, accept_len_dev);
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;

@@ -134,3 +134,24 @@ def test_turn_out_of_pages_changes_nothing_and_is_reported():
         assert spk.export(int(s))[0] == orc.export_seq(int(s))[0]
     assert np.array_equal(spk.export_refcounts(), orc.export_refcounts())
     assert orc.append(ids, ks, x["kd"], x["vd"], check=False) != 0       # the oracle refuses the same append
+
+
+def test_accept_without_the_turns_drafts_is_refused():
+    """spork_turn_accept rolls back drafts the turn appended; asked to roll a sequence back below the length
+    the plans were built for, it leaves the sequence alone and reports a device error."""
+    import paper_2607_03333_b200 as sp
+    cfg = synth.CFG4.scaled(n_groups=1, prefix_len=256, suffix_lo=40, suffix_hi=40, k_draft=0)
+    wl = synth.Workload(cfg)
+    npg, ms, mp = pool_dims(wl, 64)
+    orc, spk = make_oracle(cfg, npg, ms, mp), make_spork(cfg, npg, ms, mp)
+    ids = synth.build_state(orc, wl)
+    assert np.array_equal(ids, synth.build_state(spk, wl))
+    ks = np.full(cfg.n_seqs, 8, np.int64)
+    qi = np.concatenate([[0], np.cumsum(ks)]).astype(np.int32)
+    x = _inputs(cfg, ks, 0, 0)                        # first mismatch at position 0: every draft rejected
+    turn = spk.turn(wl.group_indptr(), ids, qi)
+    turn.accept(spk._dev(x["draft"]), spk._dev(x["target"]))     # no drafts were appended by the turn
+    assert turn.sync(check=False) == sp.ERR_DEVICE
+    assert_lens = [spk.export(int(s))[0] for s in ids]
+    assert assert_lens == [orc.export_seq(int(s))[0] for s in ids]
+    assert np.array_equal(spk.export_refcounts(), orc.export_refcounts())
