@@ -176,13 +176,12 @@ __global__ void __launch_bounds__(256) append_copy_kernel(
 // The decode loop's append (Algorithm 1 step 5: one token per live stream and step): few tokens per
 // request and no sequence twice in the batch -> ONE kernel, one block per request: take the pages,
 // publish the length, then write this request's K/V rows (its table entries are its own block's).
-__global__ void __launch_bounds__(128) append_small_kernel(
-    const AppendDesc *__restrict__ descs, const int32_t *__restrict__ free_list, int32_t *refcount,
+__device__ __forceinline__ void append_small_body(
+    const AppendDesc d, const int32_t *__restrict__ free_list, int32_t *refcount,
     int32_t *table, int table_stride, int32_t *len, int32_t *counters, int need,
     const uint4 *__restrict__ k_src, const uint4 *__restrict__ v_src, uint8_t *__restrict__ k_pool,
     uint8_t *__restrict__ v_pool, int Hkv, int chunks_per_row, int swizzled, size_t head_block) {
     __shared__ int32_t s_page[8];                 // pages of positions old_len .. (<= 64 tokens: <= 5 pages)
-    const AppendDesc d = descs[blockIdx.x];
     int32_t *row = table + (size_t)d.seq * table_stride;
     const int first_new = pages_of(d.old_len), p0 = d.old_len / PS;
     const int n_touch = d.n_tok > 0 ? (d.old_len + d.n_tok - 1) / PS - p0 + 1 : 0;
@@ -214,6 +213,30 @@ __global__ void __launch_bounds__(128) append_small_kernel(
         *reinterpret_cast<uint4 *>(k_pool + dst) = k_src[src];
         *reinterpret_cast<uint4 *>(v_pool + dst) = v_src[src];
     }
+}
+
+__global__ void __launch_bounds__(128) append_small_kernel(
+    const AppendDesc *__restrict__ descs, const int32_t *__restrict__ free_list, int32_t *refcount,
+    int32_t *table, int table_stride, int32_t *len, int32_t *counters, int need,
+    const uint4 *__restrict__ k_src, const uint4 *__restrict__ v_src, uint8_t *__restrict__ k_pool,
+    uint8_t *__restrict__ v_pool, int Hkv, int chunks_per_row, int swizzled, size_t head_block) {
+    append_small_body(descs[blockIdx.x], free_list, refcount, table, table_stride, len, counters, need, k_src, v_src,
+                      k_pool, v_pool, Hkv, chunks_per_row, swizzled, head_block);
+}
+
+// the same with the descriptors of a small batch passed as kernel PARAMETERS: the decode loop's append needs
+// no host-to-device copy at all (one launch; 3 us of a 12 us call)
+constexpr int APPEND_PARAM_MAX = 96;              // 96 x 32 B = 3 KiB of the 4 KiB parameter space
+struct AppendDescPack {
+    AppendDesc d[APPEND_PARAM_MAX];
+};
+__global__ void __launch_bounds__(128) append_small_param_kernel(
+    const __grid_constant__ AppendDescPack pack, const int32_t *__restrict__ free_list, int32_t *refcount,
+    int32_t *table, int table_stride, int32_t *len, int32_t *counters, int need,
+    const uint4 *__restrict__ k_src, const uint4 *__restrict__ v_src, uint8_t *__restrict__ k_pool,
+    uint8_t *__restrict__ v_pool, int Hkv, int chunks_per_row, int swizzled, size_t head_block) {
+    append_small_body(pack.d[blockIdx.x], free_list, refcount, table, table_stride, len, counters, need, k_src, v_src,
+                      k_pool, v_pool, Hkv, chunks_per_row, swizzled, head_block);
 }
 
 // ---- fork ------------------------------------------------------------------
@@ -449,10 +472,15 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
     int rc = ensure_pages(c, need, st);
     if (rc != SPORK_OK) return rc;
 
-    StageSlot *slot;
-    rc = stage_acquire(c, sizeof(AppendDesc) * (size_t)n, &slot);
-    if (rc != SPORK_OK) return rc;
-    AppendDesc *d = (AppendDesc *)slot->h;
+    // a small batch (the decode loop) carries its descriptors in the kernel parameters; others stage them
+    AppendDescPack pack;
+    StageSlot *slot = nullptr;
+    AppendDesc *d = pack.d;
+    if (n > APPEND_PARAM_MAX) {
+        rc = stage_acquire(c, sizeof(AppendDesc) * (size_t)n, &slot);
+        if (rc != SPORK_OK) return rc;
+        d = (AppendDesc *)slot->h;
+    }
     for (int i = 0; i < n; ++i) c->h_scratch[seq_ids[i]] = -1;  // marks "last request not yet seen"
     int fl_off = 0;
     rc = take_free(c, (int)need, st, &fl_off);
@@ -481,6 +509,22 @@ extern "C" int spork_append(spork_ctx *c, int n, const int32_t *seq_ids, const i
         foff += d[i].n_new;
         c->h_len[s] = nl;
         lineage_grow(c, s, pages_of(nl));
+    }
+    if (small && !slot) {
+        append_small_param_kernel<<<n, 128, 0, st>>>(
+            pack, c->d_free_list, c->d_refcount, c->d_table, c->table_stride, c->d_len, c->d_counters, (int)need,
+            (const uint4 *)k_src, (const uint4 *)v_src, (uint8_t *)c->k_pool, (uint8_t *)c->v_pool,
+            c->cfg.num_kv_heads, c->cfg.head_dim * c->elt / 16, c->swizzled, c->head_block);
+        c->last_launches++;
+        SPORK_CUDA(cudaGetLastError());
+        c->free_lb -= need;
+        c->len_epoch++;
+        return SPORK_OK;
+    }
+    if (!slot) {        // few requests but not the one-kernel shape (a repeated sequence, a long request): stage after all
+        rc = stage_acquire(c, sizeof(AppendDesc) * (size_t)n, &slot);
+        if (rc != SPORK_OK) return rc;
+        memcpy(slot->h, pack.d, sizeof(AppendDesc) * (size_t)n);
     }
     rc = stage_commit(c, slot, sizeof(AppendDesc) * (size_t)n, st);
     if (rc != SPORK_OK) return rc;
