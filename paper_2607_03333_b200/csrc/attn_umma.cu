@@ -84,13 +84,13 @@ struct Cfg {
     static constexpr int B_EMPTY = NSLOT;             // [NSLOT] MMAs (F8: converters) reading the slot completed
     static constexpr int B_PIPE = 2 * NSLOT;          // per pipe: 7 barriers, see P_*
     static constexpr int B_QFULL = B_PIPE + 7 * NP;   // Q staged
-    static constexpr int B_OPER = B_QFULL + 1;        // F8: V operand slot b full [2], empty [2]
-    static constexpr int B_COUNT = B_OPER + (F8 ? 4 : 0);
+    static constexpr int B_OPER = B_QFULL + 1;        // F8: V operand slot b empty [2] ("full" arrives on P_PFULL + b)
+    static constexpr int B_COUNT = B_OPER + (F8 ? 2 : 0);
     static constexpr int XCH_OFF = BAR_OFF + 8 * B_COUNT + 16;     // float [2][2][128] (SP = 2)
     static constexpr int QEXP_OFF = XCH_OFF + (SP == 2 ? 2048 : 0);   // F8: uint8 [2][128], per-row power-of-two Q scaling
     static constexpr int SMEM_BYTES = QEXP_OFF + (F8 ? 256 : 0);
 };
-enum : int { O_VFULL = 0, O_VEMPTY = 2 };
+enum : int { O_VEMPTY = 0 };
 enum : int {
     P_SFULL = 0,    // [2] S(b) complete
     P_PFULL = 2,    // [2] P(b) written (4 softmax warps)
@@ -137,17 +137,16 @@ attn_umma_kernel(const UParams P) {
         for (int w = 0; w < NP; ++w) {
             for (int b = 0; b < 2; ++b) {
                 mbar_init(pbar(w, P_SFULL + b), 1);
-                mbar_init(pbar(w, P_PFULL + b), 4 * SP);
+                mbar_init(pbar(w, P_PFULL + b), 4 * SP + (F8 ? 2 : 0));   // F8: + the two V converter warps (see below)
                 mbar_init(pbar(w, P_PVDONE + b), 1);
             }
             mbar_init(pbar(w, P_OFREE), 4 * SP);
         }
         mbar_init(bar(C::B_QFULL), 1);
         if constexpr (F8) {
-            for (int b = 0; b < 2; ++b) {
-                mbar_init(bar(C::B_OPER + O_VFULL + b), 2);     // one arrival per converter warp
-                mbar_init(bar(C::B_OPER + O_VEMPTY + b), 1);    // tcgen05.commit
-            }
+            // V operand slot b is "full" on P_PFULL + b together with P(b): tile T uses S/P buffer T & 1 AND V slot
+            // T & 1, and the MMA warp needs both before P V -- one wait instead of two (a wait costs ~190 clocks)
+            for (int b = 0; b < 2; ++b) mbar_init(bar(C::B_OPER + O_VEMPTY + b), 1);    // tcgen05.commit
         }
         mbar_fence_init();
     }
@@ -272,7 +271,7 @@ attn_umma_kernel(const UParams P) {
                 const uint32_t ldv = 2 * (gt + i) + 1;
                 // F8: tile T's V sits in operand slot T & 1, filled by the converter warps
                 const uint32_t slot = F8 ? (gt + i) & 1 : ldv % NSLOT, ph = F8 ? ((gt + i) >> 1) & 1 : (ldv / NSLOT) & 1;
-                const uint32_t v_full = F8 ? bar(C::B_OPER + O_VFULL + slot) : bar(C::B_FULL + slot);
+                const uint32_t v_full = bar(C::B_FULL + slot);      // (F8: V's readiness arrives on P_PFULL)
                 const uint32_t v_empty = F8 ? bar(C::B_OPER + O_VEMPTY + slot) : bar(C::B_EMPTY + slot);
                 const uint64_t vd = smem_desc_advance(v_desc, slot * SLOT_BYTES);
                 const int nvp = pages_of_tile(i);
@@ -281,7 +280,7 @@ attn_umma_kernel(const UParams P) {
                     if (w < npipe) {
                         const uint32_t g = g0[w] + i, b = g & 1;
                         mbar_wait(pbar(w, P_PFULL + b), (g >> 1) & 1);
-                        if (w == 0) mbar_wait(v_full, ph);
+                        if (!F8 && w == 0) mbar_wait(v_full, ph);
                         if (i == 0 && jw[w] > 0) mbar_wait(pbar(w, P_OFREE), (jw[w] - 1) & 1);
                         tc_fence_after();
                         const uint32_t tO = tbase + w * PIPE_COLS;
@@ -358,7 +357,7 @@ attn_umma_kernel(const UParams P) {
                 }
                 fence_async_smem();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar(C::B_OPER + O_VFULL + vb));
+                if (lane == 0) mbar_arrive(pbar(0, P_PFULL + vb));
             }
         }
     } else {
