@@ -473,21 +473,33 @@ class Turn:
 
     def append(self, which: int, k, v):
         """which = 0: the k_i drafts of every sequence ([sum k][Hkv][D]); 1: one token each ([n][Hkv][D])."""
-        self.spk._chk(self.spk.lib.spork_turn_append(self._t, int(which), C.c_void_p(k.data_ptr()),
-                                                      C.c_void_p(v.data_ptr()), self.spk._st))
+        self.spk._enter()        # (no-ops under torch.cuda.graph(stream=spk.stream): that IS the current stream)
+        rc = self.spk.lib.spork_turn_append(self._t, int(which), C.c_void_p(k.data_ptr()), C.c_void_p(v.data_ptr()),
+                                            self.spk._st)
+        self.spk._leave()
+        self.spk._chk(rc)
 
     def verify(self, q, out, lse):
-        self.spk._chk(self.spk.lib.spork_turn_verify(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
-                                                      C.c_void_p(lse.data_ptr()), self.spk._st))
+        self.spk._enter()
+        rc = self.spk.lib.spork_turn_verify(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
+                                            C.c_void_p(lse.data_ptr()), self.spk._st)
+        self.spk._leave()
+        self.spk._chk(rc)
 
     def accept(self, draft_tokens, target_tokens, accept_len=None):
         a = C.c_void_p(accept_len.data_ptr()) if accept_len is not None else None
-        self.spk._chk(self.spk.lib.spork_turn_accept(self._t, C.c_void_p(draft_tokens.data_ptr()),
-                                                      C.c_void_p(target_tokens.data_ptr()), a, self.spk._st))
+        self.spk._enter()
+        rc = self.spk.lib.spork_turn_accept(self._t, C.c_void_p(draft_tokens.data_ptr()),
+                                            C.c_void_p(target_tokens.data_ptr()), a, self.spk._st)
+        self.spk._leave()
+        self.spk._chk(rc)
 
     def decode(self, q, out, lse):
-        self.spk._chk(self.spk.lib.spork_turn_decode(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
-                                                      C.c_void_p(lse.data_ptr()), self.spk._st))
+        self.spk._enter()
+        rc = self.spk.lib.spork_turn_decode(self._t, C.c_void_p(q.data_ptr()), C.c_void_p(out.data_ptr()),
+                                            C.c_void_p(lse.data_ptr()), self.spk._st)
+        self.spk._leave()
+        self.spk._chk(rc)
 
     def sync(self, check: bool = True) -> int:
         """Host mirror of the lengths <- device (synchronises); the other Spork calls work again."""
