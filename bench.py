@@ -185,9 +185,20 @@ def cpu_baseline_attn(cfg, wl, ub, max_groups=0):
         ostep()
         reps += 1
     dt = (time.perf_counter() - t0) / reps
-    return {"value": ub / (dt / frac) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
-            "sample": sample + f", {reps} repetition(s)", "sample_seconds": dt * reps,
-            "scaled_ms_per_step": dt / frac * 1e3}
+    rec = {"value": ub / (dt / frac) / 1e9, "unit": "GB/s", "cores": cores, "kind": "oracle",
+           "sample": sample + f", {reps} repetition(s)", "sample_seconds": dt * reps,
+           "scaled_ms_per_step": dt / frac * 1e3}
+    if cfg.cfg_no <= 2:
+        # configs 1-2 also on ONE thread (one repetition of the same sample)
+        import oracle
+        oracle.set_num_threads(1)
+        t0 = time.perf_counter()
+        ostep()
+        d1 = time.perf_counter() - t0
+        oracle.set_num_threads(cores)
+        rec["one_thread"] = {"value": ub / (d1 / frac) / 1e9, "unit": "GB/s", "cores": 1,
+                             "scaled_ms_per_step": d1 / frac * 1e3, "sample_seconds": d1}
+    return rec
 
 
 def parity_spot_check(cfg, wl, out_np, lse_np, n_rows=2, seed=0):
@@ -624,6 +635,15 @@ def measure_cfg1(env: Env):
         rec["cpu_baseline"] = {"value": ub / dt / 1e9, "unit": "GB/s", "cores": oracle.num_threads(),
                                "kind": "oracle", "sample": "the whole step, 20 repetitions",
                                "scaled_ms_per_step": dt * 1e3}
+        cores = oracle.num_threads()
+        oracle.set_num_threads(1)
+        t0 = time.perf_counter()
+        for _ in range(20):
+            o.decode(oids, q_np)
+        d1 = (time.perf_counter() - t0) / 20
+        oracle.set_num_threads(cores)
+        rec["cpu_baseline"]["one_thread"] = {"value": ub / d1 / 1e9, "unit": "GB/s", "cores": 1,
+                                             "scaled_ms_per_step": d1 * 1e3}
     spk.close()
     return rec
 

@@ -67,6 +67,7 @@ def lib():
             "oracle_attend_dense": ([I, I, D, P, P, P, I, P, P], I),
             "oracle_widen": ([I, P, C.c_long, P], None),
             "oracle_num_threads": ([], I),
+            "oracle_set_num_threads": ([I], None),
         }
         for name, (args, res) in sig.items():
             f = getattr(_lib, name)
@@ -247,6 +248,11 @@ def attend_dense(dtype: str, scale: float, q_row: np.ndarray, K: np.ndarray, V: 
     if rc != OK:
         raise OracleError(rc)
     return out, float(lse[0])
+
+
+def set_num_threads(n: int) -> None:
+    """Threads of the oracle's OpenMP loops (bench.py's single-thread baseline; results do not depend on it)."""
+    lib().oracle_set_num_threads(int(n))
 
 
 def widen(dtype: str, a: np.ndarray) -> np.ndarray:

@@ -513,6 +513,16 @@ void oracle_widen(int dtype, const void *src, long n, double *out) {
     for (i = 0; i < n; ++i) out[i] = load_elt(&tmp, (const uint8_t *)src, (size_t)i);
 }
 
+/* threads the OpenMP loops above may use (timing only: bench.py's single-thread baseline) */
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    extern void omp_set_num_threads(int);
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int oracle_num_threads(void) {
 #ifdef _OPENMP
     extern int omp_get_max_threads(void);
