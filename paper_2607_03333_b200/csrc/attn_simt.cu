@@ -130,20 +130,32 @@ __global__ void __launch_bounds__(SIMT_WARPS * 32) attn_simt_kernel(
             for (int i = 0; i < NACC; ++i) acc[i] *= alpha;
             m = m_new;
             const int nt = min(32, it.tok1 - tb);
-            for (int tt = 0; tt < nt; ++tt) {
-                const float pt = __shfl_sync(0xffffffffu, p, tt);
-                const unsigned long long b = __shfl_sync(0xffffffffu, (unsigned long long)blk, tt);
-                if (pt == 0.f) continue;        // warp-uniform; also keeps 0 * garbage out
-                const uint8_t *vp = v_pool + b;
-                const int rr = (tb + tt) % PS;
+            // value pass: 8 tokens' V elements are requested before the first is used (each is a dependent
+            // global load: one at a time, the 32 tokens of a chunk cost 32 memory latencies)
+            for (int t0 = 0; t0 < nt; t0 += 8) {
+                float pt[8], vv[8][NACC];
 #pragma unroll
-                for (int i = 0; i < NACC; ++i) {
-                    int d = lane + 32 * i;
-                    if (d < D) {
-                        int off = chunk_off(swizzled, cpr, rr, d / E) + (d % E) * (int)sizeof(T);
-                        acc[i] = fmaf(pt, Elt<T>::load(vp + off), acc[i]);
+                for (int u = 0; u < 8; ++u) {
+                    const int tt = t0 + u;                                   // (tt < 32 always: nt <= 32, t0 % 8 == 0)
+                    pt[u] = __shfl_sync(0xffffffffu, p, tt & 31);
+                    const unsigned long long b = __shfl_sync(0xffffffffu, (unsigned long long)blk, tt & 31);
+                    if (tt >= nt) pt[u] = 0.f;
+                    const uint8_t *vp = v_pool + b;
+                    const int rr = (tb + tt) % PS;
+#pragma unroll
+                    for (int i = 0; i < NACC; ++i) {
+                        const int d = lane + 32 * i;
+                        vv[u][i] = 0.f;
+                        if (pt[u] != 0.f && d < D) {        // p = 0: masked or beyond the range -- keeps 0 * garbage out
+                            const int off = chunk_off(swizzled, cpr, rr, d / E) + (d % E) * (int)sizeof(T);
+                            vv[u][i] = Elt<T>::load(vp + off);
+                        }
                     }
                 }
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+#pragma unroll
+                    for (int i = 0; i < NACC; ++i) acc[i] = fmaf(pt[u], vv[u][i], acc[i]);
             }
         }
         const size_t prow = (size_t)it.part_base + r;
