@@ -109,6 +109,10 @@ constexpr int GROW_WINDOW = 64;                // tokens a sequence may grow bef
 constexpr int MIN_LEVEL_SAVING = 128;          // a deeper cascade level must save at least this many token reads
 constexpr float ITEM_FIXED_COST = 1.5f;        // per-item overhead in 64-token-tile times
 constexpr float ITEM_FIXED_COST_UMMA = 4.f;    // ... of the tcgen05 kernel (32 KiB of Q, 64 KiB of partials)
+// ... of its FP8-KV variant, whose tile is shorter and whose Q staging (two e4m3 terms) is longer.  Sweep on the
+// e4m3 configs (us per step at 2 / 4 / 6 / 8 / 12): config 5: 227 / 238 / 213 / 213 / 219, config 3: 241 / 192 /
+// 193 / 195 / 203, config 2: 64 / 59 / 62 / 63 / 66.  (The same sweep on bf16: 3 and 4 within 1 %, 1 and 2 far off.)
+constexpr float ITEM_FIXED_COST_UMMA_F8 = 6.f;
 // ... of a tcgen05 item in the chunked schedule, which serves the many-row (compute-heavy) verify
 // plans (sweep of the chunk length on config 4, k = 16: 630 / 587 / 650 / 669 us at 1 / 2 / 3 / 4 splits)
 constexpr float ITEM_FIXED_COST_UMMA_CHUNKED = 8.f;
@@ -529,7 +533,7 @@ int build_plan(spork_ctx *c, int n_groups, const int32_t *group_indptr, const in
         const int n_gangs = (int)std::min<int64_t>(std::max(1, grid_cap_umma / Hkv),
                                                   std::max<int64_t>(1, tiles_total / MIN_CHUNK_TILES));
         const int G_ = n_gangs * Hkv;
-        const double c0 = ITEM_FIXED_COST_UMMA;
+        const double c0 = f8 ? ITEM_FIXED_COST_UMMA_F8 : ITEM_FIXED_COST_UMMA;
         const double budget = ((double)tiles_total + c0 * ((double)order.size() + n_gangs)) / n_gangs;
         std::vector<std::vector<WorkItem>> per_cta(G_);
         int gang = 0;
