@@ -58,6 +58,7 @@ extern "C" {
 #define SPORK_ERR_CUDA (-7)         /* a CUDA runtime call failed                  */
 #define SPORK_ERR_DEVICE (-8)       /* device-side consistency check tripped       */
 #define SPORK_ERR_STALE (-9)        /* a captured turn ran: call spork_turn_sync    */
+#define SPORK_ERR_LIMIT (-10)       /* size beyond a no-allocation entry point's fixed maximum */
 
 #define SPORK_F32 0
 #define SPORK_BF16 1
@@ -262,6 +263,34 @@ int spork_accept(spork_ctx *ctx, int n, const int32_t *seq_ids, const int32_t *q
  */
 int spork_confidence(spork_ctx *ctx, int n_spans, const int32_t *span_indptr, const float *logits,
                      int vocab, float *confidence_out, void *stream);
+
+/*
+ * The same score (Eq. 2) for callers that cannot allocate: code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc.  The call makes two kernel launches
+ * on `stream` and nothing else -- no cudaMalloc / cudaFree or allocating library routine, no staging
+ * copy, no synchronisation, no host read of device memory -- and needs no context.  The per-(row,
+ * vocabulary slice) partial sums that spork_confidence keeps in a buffer it grows live here in ONE
+ * file-scope device array of 2 * SPORK_CONFIDENCE_STATIC_MAX_ROWS float2 (256 KiB), which every GPU
+ * that loads libspork holds until the process exits.
+ *   span_indptr    DEVICE int32[n_spans + 1] (spork_confidence reads it on the host): non-decreasing,
+ *                  span_indptr[0] = 0, span_indptr[n_spans] = n_pos.  Not checked (it is device memory);
+ *                  values outside this contract give undefined scores and may read outside the array.
+ *   n_pos          rows of logits; at most SPORK_CONFIDENCE_STATIC_MAX_ROWS, else SPORK_ERR_LIMIT and
+ *                  nothing is launched.
+ *   logits         DEVICE fp32 [n_pos][vocab], row-major; confidence_out: DEVICE fp32[n_spans].
+ * Results equal spork_confidence's up to the rounding of a different slicing of the vocabulary.
+ * The array is shared by every call on the device and keeps the last call's contents: each slot a call
+ * reads it has written itself (nothing needs to start at zero), but two calls that OVERLAP on the GPU
+ * (different streams, parallel graph branches) race on it -- order them.  The first call on a device
+ * resolves the array's device address (cudaGetSymbolAddress, with that device current) and must be
+ * made outside stream capture; n_spans = 0 does only that.  The current device must be the one
+ * `stream`, the pointers and later calls belong to.  Errors: SPORK_ERR_INVALID (null pointers,
+ * negative sizes, vocab < 1), SPORK_ERR_LIMIT (n_pos beyond the maximum, device ordinal >= 64),
+ * SPORK_ERR_CUDA.
+ */
+#define SPORK_CONFIDENCE_STATIC_MAX_ROWS 16384
+int spork_confidence_static(int n_spans, const int32_t *span_indptr, int n_pos, const float *logits,
+                            int vocab, float *confidence_out, void *stream);
 
 /*
  * Tuning knob of the planner (bf16, D = 128 contexts only): a segment -- a fork group's shared

@@ -24,6 +24,8 @@ PAGE_SIZE = 16
 
 OK = 0
 ERR_STALE = -9
+ERR_LIMIT = -10
+CONFIDENCE_STATIC_MAX_ROWS = 16384
 ERR_INVALID, ERR_OOM, ERR_NO_SLOT, ERR_TOO_LONG, ERR_INVALID_SEQ, ERR_SHARED, ERR_CUDA, ERR_DEVICE = (
     -1, -2, -3, -4, -5, -6, -7, -8)
 
@@ -37,7 +39,7 @@ ABI_SYMBOLS = [
     "spork_set_cascade_levels", "spork_layers", "spork_write_kv_layer", "spork_decode_attn_layers",
     "spork_verify_attn_layers", "spork_hbm_read_probe",
     "spork_turn_prepare", "spork_turn_append", "spork_turn_verify", "spork_turn_accept", "spork_turn_decode",
-    "spork_turn_sync", "spork_turn_destroy",
+    "spork_turn_sync", "spork_turn_destroy", "spork_confidence_static",
 ]
 
 
@@ -98,6 +100,7 @@ def load(build_if_missing: bool = True):
         "spork_last_launches": ([P], I),
         "spork_accept": ([P, I, P, P, P, P, P, P], I),
         "spork_confidence": ([P, I, P, P, I, P, P], I),
+        "spork_confidence_static": ([I, P, I, P, I, P, P], I),
         "spork_set_timing": ([P, I], I),
         "spork_set_tensor_path_min_rows": ([P, I], I),
         "spork_set_many_row_variant": ([P, I], I),
@@ -287,6 +290,25 @@ class Spork:
         self._hold(x, out)
         self._chk(rc, check)
         return out if check else (rc, out)
+
+    def confidence_static(self, span_indptr, logits, out, check: bool = True):
+        """spork_confidence_static: Eq. 2 confidence with no allocation anywhere (see spork.h).  All three
+        arguments are device tensors the caller owns: span_indptr int32 [n_spans + 1], logits fp32
+        [n_pos][vocab] (at most CONFIDENCE_STATIC_MAX_ROWS rows), out fp32 [n_spans].  Runs on this
+        context's stream; returns the error code."""
+        torch = self.torch
+        assert span_indptr.dtype == torch.int32 and span_indptr.is_cuda and span_indptr.is_contiguous()
+        assert logits.dtype == torch.float32 and logits.is_cuda and logits.is_contiguous() and logits.dim() == 2
+        n = int(span_indptr.numel()) - 1
+        assert out.dtype == torch.float32 and out.is_cuda and out.is_contiguous() and out.numel() == n
+        self._enter()
+        with torch.cuda.device(self.device):       # the call resolves its scratch on the CURRENT device
+            rc = self.lib.spork_confidence_static(n, C.c_void_p(span_indptr.data_ptr()), int(logits.shape[0]),
+                                                  C.c_void_p(logits.data_ptr()), int(logits.shape[1]),
+                                                  C.c_void_p(out.data_ptr()), self._st)
+        self._leave()
+        self._hold(span_indptr, logits, out)
+        return self._chk(rc, check)
 
     def turn(self, group_indptr, seq_ids, q_indptr) -> "Turn":
         """Prepares a capturable partial-token-accept turn over this batch (see spork.h, spork_turn_*)."""

@@ -82,6 +82,7 @@ extern "C" const char *spork_strerror(int code) {
         case SPORK_ERR_CUDA: return "CUDA runtime error";
         case SPORK_ERR_DEVICE: return "device-side consistency check failed";
         case SPORK_ERR_STALE: return "host lengths are stale after a captured turn: call spork_turn_sync";
+        case SPORK_ERR_LIMIT: return "size beyond the fixed maximum of a no-allocation entry point";
         default: return "unknown spork error";
     }
 }

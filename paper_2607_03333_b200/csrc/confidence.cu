@@ -11,6 +11,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "spork_internal.h"
 
@@ -181,6 +182,135 @@ extern "C" int spork_confidence(spork_ctx *c, int n_spans, const int32_t *span_i
     conf_span_kernel<<<ceil_div(n_spans, 4), 128, 0, st>>>(d_span, n_spans, (const float2 *)c->ws_conf.p, splits,
                                                            confidence_out);
     c->last_launches++;
+    SPORK_CUDA(cudaGetLastError());
+    return SPORK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// spork_confidence_static: the same score for callers that cannot allocate (CUDA-graph capture, tight
+// serving loops).  The per-(row, slice) partials live in a file-scope device array instead of the
+// context's grown buffer, and the spans are read from DEVICE memory, so the call is two launches and
+// nothing else: no cudaMalloc / cudaFree, no staging copy, no host read of device memory.
+//   conf_partial_static_kernel : conf_partial_kernel without the row list -- CTA (row, slice) finds out
+//                                from the device span_indptr whether its row opens a span (Eq. 2 skips
+//                                i = 1) and leaves if so
+//   conf_span_kernel           : as above, over the static array
+// Every GPU that loads libspork holds the array (256 KiB) until the process exits.  All calls share it:
+// a slot the span kernel reads is written by the partial kernel of the same call (nothing has to start
+// at zero, stale contents of earlier calls are never read), but two calls that overlap on the GPU
+// (different streams, or graph branches) race on it.
+namespace {
+
+constexpr int STATIC_MAX_ROWS = SPORK_CONFIDENCE_STATIC_MAX_ROWS;
+constexpr int STATIC_MAX_PARTS = 2 * STATIC_MAX_ROWS;          // float2 each: 256 KiB
+constexpr int STATIC_MAX_DEVICES = 64;
+
+static __device__ __align__(256) float2 conf_static_scratch[STATIC_MAX_PARTS];
+
+// The array's name is a host-side stand-in in host code: the device address is resolved once per
+// device (with that device current) and kept here.
+struct StaticDev {
+    float2 *part = nullptr;
+    int num_sms = 0;
+};
+StaticDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+
+__global__ void __launch_bounds__(THREADS) conf_partial_static_kernel(const float *__restrict__ logits, int vocab,
+                                                                      int chunk, int splits, int vec,
+                                                                      const int32_t *__restrict__ span_indptr,
+                                                                      int n_spans, float2 *__restrict__ part) {
+    const int row = blockIdx.x / splits, sx = blockIdx.x % splits;
+    // the last j with span_indptr[j] <= row is the span holding the row (empty spans repeat a value)
+    int lo = 0, hi = n_spans;
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (span_indptr[mid] <= row) lo = mid; else hi = mid - 1;
+    }
+    if (span_indptr[lo] == row) return;                       // i = 1 of its span: not part of the minimum
+    const float *x = logits + (size_t)row * vocab;
+    const int v0 = sx * chunk, v1 = min(vocab, v0 + chunk);
+    float m = -INFINITY, s = 0.f;
+    if (vec) {
+        constexpr int NB = 4;
+        for (int v = v0 + threadIdx.x * 8; v < v1; v += THREADS * 8 * NB) {
+            float t[NB][8];
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const int vk = v + k * THREADS * 8;
+                if (vk + 8 <= v1) {
+                    const float4 a = __ldcs(reinterpret_cast<const float4 *>(x + vk));
+                    const float4 b = __ldcs(reinterpret_cast<const float4 *>(x + vk + 4));
+                    t[k][0] = a.x; t[k][1] = a.y; t[k][2] = a.z; t[k][3] = a.w;
+                    t[k][4] = b.x; t[k][5] = b.y; t[k][6] = b.z; t[k][7] = b.w;
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) t[k][i] = vk + i < v1 ? x[vk + i] : -INFINITY;
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NB; ++k) absorb8(m, s, t[k]);
+        }
+    } else {
+        for (int v = v0 + threadIdx.x * 8; v < v1; v += THREADS * 8) {
+            float t[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) t[i] = v + i < v1 ? x[v + i] : -INFINITY;
+            absorb8(m, s, t);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+        combine(m, s, __shfl_xor_sync(0xffffffffu, m, o), __shfl_xor_sync(0xffffffffu, s, o));
+    __shared__ float2 red[THREADS / 32];
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = make_float2(m, s);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < THREADS / 32; ++w) combine(m, s, red[w].x, red[w].y);
+        part[(size_t)row * splits + sx] = make_float2(m, s);
+    }
+}
+
+}  // namespace
+
+extern "C" int spork_confidence_static(int n_spans, const int32_t *span_indptr, int n_pos, const float *logits,
+                                       int vocab, float *confidence_out, void *stream) {
+    if (n_spans < 0 || n_pos < 0 || vocab < 1) return SPORK_ERR_INVALID;
+    if (n_pos > STATIC_MAX_ROWS) return SPORK_ERR_LIMIT;
+    int dev = -1;
+    SPORK_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return SPORK_ERR_LIMIT;
+    StaticDev sd;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_dev[dev].part) {          // set-up, once per device, that device current
+            float2 *p = nullptr;
+            int sms = 0;
+            SPORK_CUDA(cudaGetSymbolAddress((void **)&p, conf_static_scratch));
+            SPORK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            if (!p || sms < 1) return SPORK_ERR_CUDA;
+            g_static_dev[dev].num_sms = sms;
+            g_static_dev[dev].part = p;
+        }
+        sd = g_static_dev[dev];
+    }
+    if (n_spans == 0) return SPORK_OK;          // (a set-up call: the address is resolved, nothing runs)
+    if (!span_indptr || !confidence_out || (n_pos > 0 && !logits)) return SPORK_ERR_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    int splits = 1, chunk = THREADS * 8;
+    if (n_pos > 0) {
+        // as spork_confidence (>= 8 CTAs per SM; the CTAs of span-opening rows leave at once), then what
+        // the array holds: at least 2 slices per row
+        splits = ceil_div(8 * sd.num_sms, n_pos);
+        splits = std::max(1, std::min(splits, ceil_div(vocab, THREADS * 8)));
+        splits = std::min(splits, STATIC_MAX_PARTS / n_pos);
+        chunk = ceil_div(ceil_div(vocab, splits), THREADS * 8) * THREADS * 8;
+        splits = ceil_div(vocab, chunk);
+        const int vec = (vocab & 3) == 0 && ((uintptr_t)logits & 15) == 0;
+        conf_partial_static_kernel<<<(unsigned)(splits * n_pos), THREADS, 0, st>>>(logits, vocab, chunk, splits, vec,
+                                                                                   span_indptr, n_spans, sd.part);
+    }
+    conf_span_kernel<<<ceil_div(n_spans, 4), 128, 0, st>>>(span_indptr, n_spans, sd.part, splits, confidence_out);
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;
 }
