@@ -274,7 +274,8 @@ int spork_confidence(spork_ctx *ctx, int n_spans, const int32_t *span_indptr, co
  * that loads libspork holds until the process exits.
  *   span_indptr    DEVICE int32[n_spans + 1] (spork_confidence reads it on the host): non-decreasing,
  *                  span_indptr[0] = 0, span_indptr[n_spans] = n_pos.  Not checked (it is device memory);
- *                  values outside this contract give undefined scores and may read outside the array.
+ *                  values outside this contract give undefined scores (the kernels clamp them to the
+ *                  rows that exist: nothing outside the array or the logits is read).
  *   n_pos          rows of logits; at most SPORK_CONFIDENCE_STATIC_MAX_ROWS, else SPORK_ERR_LIMIT and
  *                  nothing is launched.
  *   logits         DEVICE fp32 [n_pos][vocab], row-major; confidence_out: DEVICE fp32[n_spans].

@@ -194,7 +194,7 @@ extern "C" int spork_confidence(spork_ctx *c, int n_spans, const int32_t *span_i
 //   conf_partial_static_kernel : conf_partial_kernel without the row list -- CTA (row, slice) finds out
 //                                from the device span_indptr whether its row opens a span (Eq. 2 skips
 //                                i = 1) and leaves if so
-//   conf_span_kernel           : as above, over the static array
+//   conf_span_static_kernel    : conf_span_kernel over the static array, span bounds clamped to the rows
 // Every GPU that loads libspork holds the array (256 KiB) until the process exits.  All calls share it:
 // a slot the span kernel reads is written by the partial kernel of the same call (nothing has to start
 // at zero, stale contents of earlier calls are never read), but two calls that overlap on the GPU
@@ -271,6 +271,29 @@ __global__ void __launch_bounds__(THREADS) conf_partial_static_kernel(const floa
     }
 }
 
+// conf_span_kernel with the span bounds clamped to [0, n_pos]: the spans come from device memory here and
+// cannot be validated on the host, so a bad span_indptr gives wrong scores, never a read outside the array
+__global__ void __launch_bounds__(128) conf_span_static_kernel(const int32_t *__restrict__ span_indptr, int n_spans,
+                                                               int n_pos, const float2 *__restrict__ part, int splits,
+                                                               float *__restrict__ conf) {
+    const int w = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (w >= n_spans) return;
+    const int r0 = max(0, span_indptr[w]), r1 = min(n_pos, span_indptr[w + 1]);
+    float c = 1.f;                                           // empty minimum (A-23)
+    for (int row = r0 + 1; row < r1; ++row) {                // i = 2 .. L
+        float m = -INFINITY, s = 0.f;
+        for (int k = lane; k < splits; k += 32) {
+            const float2 p = part[(size_t)row * splits + k];
+            combine(m, s, p.x, p.y);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+            combine(m, s, __shfl_xor_sync(0xffffffffu, m, o), __shfl_xor_sync(0xffffffffu, s, o));
+        c = fminf(c, 1.f / s);
+    }
+    if (lane == 0) conf[w] = c;
+}
+
 }  // namespace
 
 extern "C" int spork_confidence_static(int n_spans, const int32_t *span_indptr, int n_pos, const float *logits,
@@ -310,7 +333,8 @@ extern "C" int spork_confidence_static(int n_spans, const int32_t *span_indptr, 
         conf_partial_static_kernel<<<(unsigned)(splits * n_pos), THREADS, 0, st>>>(logits, vocab, chunk, splits, vec,
                                                                                    span_indptr, n_spans, sd.part);
     }
-    conf_span_kernel<<<ceil_div(n_spans, 4), 128, 0, st>>>(span_indptr, n_spans, sd.part, splits, confidence_out);
+    conf_span_static_kernel<<<ceil_div(n_spans, 4), 128, 0, st>>>(span_indptr, n_spans, n_pos, sd.part, splits,
+                                                                 confidence_out);
     SPORK_CUDA(cudaGetLastError());
     return SPORK_OK;
 }

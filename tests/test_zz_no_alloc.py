@@ -83,6 +83,13 @@ def test_static_scratch_entry_point_edges_and_limit():
     out2 = torch.full((2,), -1.0, dtype=torch.float32, device=spk.device)
     assert spk.confidence_static(spk._dev(np.zeros(3, np.int32)), xd[:0], out2) == 0
     assert out2.cpu().numpy().tolist() == [1.0, 1.0]
+    # spans that break the contract (device memory, not checked): clamped to the rows that exist -- the
+    # scores mean nothing, but nothing faults and the next call is served as usual
+    bad = spk._dev(np.array([0, 10 ** 6, -5, 3], np.int32))
+    assert spk.confidence_static(bad, xd, out) == 0
+    spk.synchronize()
+    assert spk.confidence_static(spd, xd, out) == 0
+    _check(spk, (x, sp, xd, spd, out), "after a bad span_indptr")
     # one row beyond the fixed maximum: refused before anything is launched, the output is untouched
     n = sp_mod.CONFIDENCE_STATIC_MAX_ROWS + 1
     big = torch.zeros((n, 8), dtype=torch.float32, device=spk.device)
